@@ -1,0 +1,174 @@
+"""Pins P1, P10 and the threshold table: Philox, generator, colouring, thresholds.
+
+All CPU (-m "not gpu").  Citations: DESIGN.md §3 (O1-O6), SURVEY.md §8(c) P1/P10/Q13.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from tests import exact
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _kat_rows():
+    rows = []
+    for line in open(os.path.join(GOLD, "philox_kat.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        rows.append([int(x, 16) for x in line.split()])
+    return rows
+
+
+def py_philox(c, k):
+    """Second, independent statement of Philox4x32-10 with Python big ints."""
+    c = list(c)
+    k = list(k)
+    for _ in range(10):
+        p0 = 0xD2511F53 * c[0]
+        p1 = 0xCD9E8D57 * c[2]
+        c = [(p1 >> 32) ^ c[1] ^ k[0], p1 & 0xFFFFFFFF, (p0 >> 32) ^ c[3] ^ k[1], p0 & 0xFFFFFFFF]
+        k = [(k[0] + 0x9E3779B9) & 0xFFFFFFFF, (k[1] + 0xBB67AE85) & 0xFFFFFFFF]
+    return c
+
+
+def test_philox_known_answers(oracle_mod):
+    rows = _kat_rows()
+    assert len(rows) >= 11
+    for v in rows:
+        assert list(oracle_mod.philox(*v[:6])) == v[6:]
+        assert py_philox(v[:4], v[4:6]) == v[6:]
+
+
+def test_philox_random_counters_match_second_implementation(oracle_mod):
+    rng = np.random.default_rng(7)
+    for _ in range(200):
+        v = [int(x) for x in rng.integers(0, 1 << 32, size=6)]
+        assert list(oracle_mod.philox(*v)) == py_philox(v[:4], v[4:])
+
+
+def test_initial_word_matches_published_layout_vector(oracle_mod):
+    # seed 1, tag 1, site 0, word 0 -> x0|x1<<32 = 0x8c4707329f3f38ef
+    o = oracle_mod.Oracle(oracle_mod.VB, 16, 2.0, 1.0, 1, 1)
+    assert int(o.spins()[0, 0]) == 0x8C4707329F3F38EF
+    # coupling word of edge 0, word 0 (tag 2): 0x8510e6e40c19cc69
+    assert int(o.couplings()[0, 0]) == 0x8510E6E40C19CC69
+
+
+def test_threshold_table_golden(oracle_mod):
+    for line in open(os.path.join(GOLD, "thresholds.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        model, T, N, k, val = line.split()
+        T, N, k, val = float(T), int(N), int(k), int(val)
+        if model == "VB":
+            # a dense little graph so that d_max >= 4
+            o = oracle_mod.Oracle(oracle_mod.VB, 12, 8.0, T, 3, 1)
+            assert o.max_degree >= 4
+            assert int(o.thresholds(k + 1)[k]) == val
+        else:
+            pytest.importorskip("numpy")
+            # thrSK depends only on (N, T): read it off a tiny-W instance of that N is too slow to
+            # build at N=4096 (8M couplings) in the oracle?  No: 8.4M Philox calls ~ 1 s.
+            o = oracle_mod.Oracle(oracle_mod.SK, N, 0.0, T, 1, 1)
+            assert int(o.thresholds(k + 1)[k]) == val
+            if val == 0:
+                assert int(o.thresholds(k)[k - 1]) > 0  # first zero (m=426)
+
+
+def test_threshold_limits(oracle_mod):
+    o0 = oracle_mod.Oracle(oracle_mod.VB, 64, 4.0, 0.0, 1, 1)
+    assert np.all(o0.thresholds(o0.max_degree + 1) == 0)
+    oi = oracle_mod.Oracle(oracle_mod.VB, 64, 4.0, float("inf"), 1, 1)
+    assert np.all(oi.thresholds(oi.max_degree + 1)[1:] == 1 << 32)
+    # closed form, written independently
+    o = oracle_mod.Oracle(oracle_mod.VB, 64, 4.0, 1.3, 1, 1)
+    thr = o.thresholds(o.max_degree + 1)
+    for k in range(1, o.max_degree + 1):
+        assert int(thr[k]) == math.floor(math.exp(-(2.0 * k) / 1.3) * 2.0**32)
+    assert np.all(np.diff(thr[1:].astype(np.int64)) <= 0)
+
+
+@pytest.mark.parametrize("N,c,seed", [(1024, 4.0, 1), (4096, 4.0, 5), (500, 3.0, 2), (64, 6.5, 9)])
+def test_generator_structure(oracle_mod, N, c, seed):
+    o = oracle_mod.Oracle(oracle_mod.VB, N, c, 1.0, seed, 1)
+    M = math.floor(c * N / 2 + 0.5)
+    assert o.M == M
+    e = o.edges().astype(np.int64)
+    assert e.shape == (M, 2)
+    assert np.all(e[:, 0] != e[:, 1])                              # no self-loops
+    key = np.minimum(e[:, 0], e[:, 1]) * N + np.maximum(e[:, 0], e[:, 1])
+    assert len(np.unique(key)) == M                                # no multi-edges
+    assert e.min() >= 0 and e.max() < N
+    row_ptr, col, colour = o.graph()
+    deg = np.bincount(e.ravel(), minlength=N)
+    assert np.array_equal(np.diff(row_ptr.astype(np.int64)), deg)
+    # CSR rows hold exactly the neighbours
+    for i in range(0, N, max(1, N // 50)):
+        mine = sorted(col[int(row_ptr[i]):int(row_ptr[i + 1])].tolist())
+        ref = sorted(e[e[:, 0] == i, 1].tolist() + e[e[:, 1] == i, 0].tolist())
+        assert mine == ref
+    # proper colouring + first-fit property + equals an independent first-fit
+    assert np.all(colour[e[:, 0]] != colour[e[:, 1]])
+    assert np.array_equal(colour.astype(np.int64), exact.first_fit_colouring(N, e))
+    assert o.n_colours == int(colour.max()) + 1
+    assert o.max_degree == int(deg.max())
+
+
+def test_generator_follows_O2_attempt_sequence(oracle_mod):
+    """Re-derive the accepted edge list from the attempt stream with the second Philox."""
+    N, c, seed = 40, 4.0, 11
+    o = oracle_mod.Oracle(oracle_mod.VB, N, c, 1.0, seed, 1)
+    M = o.M
+    got = o.edges().tolist()
+    seen, ref, a = set(), [], 0
+    while len(ref) < M:
+        x = py_philox([a & 0xFFFFFFFF, a >> 32, 0, 3 << 24], [seed & 0xFFFFFFFF, seed >> 32])
+        u, v = (x[0] * N) >> 32, (x[1] * N) >> 32
+        a += 1
+        if u == v or (min(u, v), max(u, v)) in seen:
+            continue
+        seen.add((min(u, v), max(u, v)))
+        ref.append([u, v])
+    assert got == ref
+
+
+def test_degree_histogram_is_poisson(oracle_mod):
+    N, c = 1 << 16, 4.0
+    o = oracle_mod.Oracle(oracle_mod.VB, N, c, 1.0, 1, 1)
+    deg = np.bincount(o.edges().ravel(), minlength=N)
+    assert deg.sum() == 2 * o.M and abs(deg.mean() - c) < 1e-9
+    kmax = 12
+    obs = np.bincount(np.minimum(deg, kmax), minlength=kmax + 1).astype(float)
+    p = np.array([math.exp(-c) * c**k / math.factorial(k) for k in range(kmax)])
+    p = np.append(p, 1 - p.sum())
+    chi2 = ((obs - N * p) ** 2 / (N * p)).sum()
+    # G(N,M) degrees are multinomial (slightly under-dispersed vs Poisson): chi2 <~ dof=12
+    assert chi2 < 40.0, chi2
+    # SURVEY P10 reference values for c=4
+    ref = [.0183, .0733, .1465, .1954, .1954, .1563, .1042, .0595, .0298]
+    assert np.allclose(obs[:9] / N, ref, atol=4e-3)
+
+
+def test_bits_are_fair(oracle_mod):
+    N = 1 << 14
+    o = oracle_mod.Oracle(oracle_mod.VB, N, 4.0, 1.0, 4, 2)
+    S = exact.unpack(o.spins())                    # (N, 128)
+    frac = (S < 0).mean(axis=0)
+    assert np.all(np.abs(frac - 0.5) < 5 * 0.5 / math.sqrt(N))
+    K = exact.unpack(o.couplings())                # (M, 128)
+    frac = (K < 0).mean(axis=0)
+    assert np.all(np.abs(frac - 0.5) < 5 * 0.5 / math.sqrt(o.M))
+    # lanes are pairwise uncorrelated (independent disorder per lane)
+    cc = np.corrcoef(K[:, :16].T.astype(float))
+    off = cc[~np.eye(16, dtype=bool)]
+    assert np.abs(off).max() < 5 / math.sqrt(o.M)
+
+
+def test_create_rejects_bad_arguments(oracle_mod):
+    for args in [(0, 1, 4.0, 1.0, 1, 1), (0, 100, 4.0, 1.0, 1, 0), (0, 10, 40.0, 1.0, 1, 1),
+                 (0, 100, 4.0, -1.0, 1, 1), (2, 100, 4.0, 1.0, 1, 1), (1, 40000, 0.0, 1.0, 1, 1)]:
+        with pytest.raises(ValueError):
+            oracle_mod.Oracle(*args)
