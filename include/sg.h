@@ -1,0 +1,165 @@
+/*
+ * sg.h -- C-ABI of the B200-native multispin Monte Carlo library (libsg.so).
+ *
+ * The calls follow the paper's statement of the problem (arXiv:1906.11195):
+ *   an instance (graph + couplings + random start)
+ *   Metropolis sweeps, "update of the whole graph as unit of time", PAPER.md:260 (VB), :233 (SK)
+ *   stored configurations and the two-time correlation C(t,t')
+ *   the energy, PAPER.md:43 (Eq. 1), :73 (Eq. 3), :324
+ * and BASELINE.json's north_star call list.  All conventions (bit meanings, Philox counter
+ * layout, thresholds, colouring, schedule) are in DESIGN.md section 3.
+ *
+ * Everything runs on the current CUDA device, on torch's current CUDA stream; device
+ * memory comes from torch's caching allocator (the process must have imported torch so
+ * that libc10_cuda is loaded).  There is no CPU fallback: without a CUDA device sg_create
+ * fails.  No function aborts or throws; failures return a negative code (or NULL) and set
+ * a thread-local message readable with sg_last_error().
+ *
+ * Pointer arguments marked HOST are caller-owned host memory.  No device pointer crosses
+ * this interface.  A handle must be used by one thread at a time.
+ */
+#ifndef SG_H
+#define SG_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sg_sim sg_sim; /* opaque; owns every device and host buffer of one simulation */
+
+enum { SG_MODEL_VB = 0, SG_MODEL_SK = 1 };
+enum { SG_OK = 0, SG_EINVAL = -1, SG_ENOMEM = -2, SG_ECUDA = -3, SG_ESLOT = -4 };
+#define SG_MAX_SLOTS 64
+
+/*
+ * sg_create -- build one simulation: n_words*64 independent samples ("lanes") that share the
+ * interaction graph and differ in couplings and initial spins.
+ *   model   SG_MODEL_VB: Viana-Bray +-J model (Eq. 3) on an Erdos-Renyi graph G(N, M),
+ *                        M = floor(c*N/2 + 0.5), self-loops and multi-edges rejected (O2);
+ *           SG_MODEL_SK: Sherrington-Kirkpatrick model (Eq. 1) with binary couplings
+ *                        +-1/sqrt(N); c is ignored.
+ *   N       number of sites, 2 <= N < 2^32 (SK: N <= 32768 so that int16 local fields are exact).
+ *   c       mean degree (VB), c >= 0 and M <= N(N-1)/2.
+ *   T       temperature, 0 <= T <= +inf (T = 0 and T = inf are legal).
+ *   seed    Philox key.  (model, N, c, T, seed, n_words) determine every bit of every output.
+ *   n_words 64-bit words per site, >= 1; lane l = 64*w + b is bit b of word w.
+ * Spins start uniformly random, sweep counter = 0.
+ * Returns NULL on failure (bad argument, no CUDA device, out of memory).
+ */
+sg_sim *sg_create(int model, uint64_t N, double c, double T, uint64_t seed, uint32_t n_words);
+
+/* Release everything the handle owns (synchronises the stream first).  NULL is allowed. */
+void sg_destroy(sg_sim *h);
+
+/*
+ * sg_sweep -- advance n full Metropolis sweeps (one sweep = every site of every lane proposed once:
+ * VB colour class by colour class, SK sites 0..N-1 in order; O7/O8).  Asynchronous:
+ * kernels are enqueued on the current stream.  n = 0 is a no-op.
+ */
+int sg_sweep(sg_sim *h, uint64_t n);
+
+/*
+ * sg_snapshot -- slot <- current configuration (device-to-device copy on the stream; the slot is
+ * allocated on first use).  slot < SG_MAX_SLOTS, else SG_EINVAL.  Asynchronous.
+ */
+int sg_snapshot(sg_sim *h, uint32_t slot);
+
+/*
+ * sg_correlation -- out_counts[l] = D_l = #{ i : s_i(now) != s_i(slot) } for every lane l,
+ * so that C(tw, tw+t) = 1 - 2*D_l/N.  Exact integers.
+ *   out_counts  HOST, 64*n_words uint64.
+ * Synchronises the stream.  SG_ESLOT if the slot was never written.
+ */
+int sg_correlation(sg_sim *h, uint32_t slot, uint64_t *out_counts);
+
+/*
+ * sg_energy -- per-lane energy of the current configuration, exact integers.
+ *   VB: out[l] = E_l  = -sum_{(ij) in E} J_ij s_i s_j
+ *   SK: out[l] = E'_l = -sum_{i<j} J'_ij s_i s_j with J' = +-1; energy = E'_l / sqrt(N)
+ *   out  HOST, 64*n_words int64.
+ * Synchronises the stream.
+ */
+int sg_energy(sg_sim *h, int64_t *out);
+
+/* Message of the last failure on this thread ("" if none). */
+const char *sg_last_error(void);
+
+/* ---- debug / test getters (synchronise; not on the timed path) ------------------------------ */
+
+/* Number of sweeps done so far. */
+uint64_t sg_sweep_count(const sg_sim *h);
+/* Number of edges M (VB) or N(N-1)/2 (SK). */
+uint64_t sg_num_edges(const sg_sim *h);
+/* Number of colour classes K (VB; 0 for SK) and maximum degree (VB; N-1 for SK). */
+uint32_t sg_num_colours(const sg_sim *h);
+uint32_t sg_max_degree(const sg_sim *h);
+
+/*
+ * Spin words in ORIGINAL site order, word-minor: out[i*n_words + w], bit 1 <=> s = -1.
+ *   slot  -1 = current configuration, else a snapshot slot (SG_ESLOT if never written).
+ *   out   HOST, N*n_words uint64.
+ */
+int sg_get_spins(sg_sim *h, int32_t slot, uint64_t *out);
+
+/*
+ * Overwrite the current configuration / the sweep counter (tests: a sweep is a pure function of
+ * (configuration, sweep index), Q15).  in: HOST, N*n_words uint64, original site order.
+ */
+int sg_set_spins(sg_sim *h, const uint64_t *in);
+int sg_set_sweep_count(sg_sim *h, uint64_t t);
+
+/*
+ * VB graph in original labels: row_ptr HOST N+1 uint64, col HOST 2M uint32 (neighbours of i at
+ * col[row_ptr[i] .. row_ptr[i+1]), in increasing edge id), colour HOST N uint32.  Any may be NULL.
+ */
+int sg_get_graph(sg_sim *h, uint64_t *row_ptr, uint32_t *col, uint32_t *colour);
+/* VB edge list in generation order: u, v HOST M uint32 each. */
+int sg_get_edges(sg_sim *h, uint32_t *u, uint32_t *v);
+/*
+ * Coupling words as stored on the device, bit 1 <=> J = -1.
+ *   VB: out[e*n_words + w], edge order of generation (read back from the site-major device array).
+ *   SK: out[pair(i,j)*n_words + w], i<j row-major upper triangle.
+ *   out HOST, M*n_words uint64.
+ */
+int sg_get_couplings(sg_sim *h, uint64_t *out);
+/* Acceptance thresholds thr[0..n) as 64-bit integers (index 0 unused = 0). out HOST n uint64. */
+int sg_get_thresholds(sg_sim *h, uint64_t *out, uint64_t n);
+
+/* ---- host-only entry points (no GPU needed; tests of the host generator and host Philox) -------- */
+
+/* Philox4x32-10 block as the host generator evaluates it (O1). out HOST 4 uint32. */
+void sg_host_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1, uint32_t *out);
+
+/*
+ * The VB instance exactly as sg_create lays it out for the device, built on
+ * the host only.  Sites are relabelled to positions p sorted by (colour, degree, label); a colour class
+ * is cut into slices of 32 positions; slice g stores its rows column-major: entry 32*slice_ptr[g] + 32*k + j
+ * is the k-th neighbour (a position) of the j-th site of the slice; padding entries hold the site's own
+ * position and edge id 0xFFFFFFFF.
+ */
+typedef struct sg_host_graph sg_host_graph;
+sg_host_graph *sg_host_graph_create(uint64_t N, double c, uint64_t seed);   /* NULL on bad arguments */
+void sg_host_graph_destroy(sg_host_graph *g);
+/* info HOST 6 uint64: M, K (colours), dmax, entries, nslices, N */
+int sg_host_graph_info(const sg_host_graph *g, uint64_t *info);
+/*
+ * Copies out whichever arrays are non-NULL (all HOST): u,v M uint32; colour N uint32; orig N uint32
+ * (position -> label); deg N uint32 (per position); slice_ptr nslices+1 uint32; col entries uint32;
+ * eid entries uint32; class_pos0, class_n, class_slice0 K uint64 each.
+ */
+int sg_host_graph_get(const sg_host_graph *g, uint32_t *u, uint32_t *v, uint32_t *colour, uint32_t *orig,
+                      uint32_t *deg, uint32_t *slice_ptr, uint32_t *col, uint32_t *eid,
+                      uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0);
+
+/*
+ * Number of kernels this library has launched (process-wide, all handles) since load.
+ * bench.py reports the difference over its timed region as "gpu_launches".
+ */
+uint64_t sg_kernel_launches(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SG_H */

@@ -1,0 +1,272 @@
+// sg_api.cu -- the C-ABI of include/sg.h: handle, argument checks, buffer ownership, call
+// sequencing.  Every step of the path runs in the kernels of sg_kernels.cu / sg_sk.cu.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstring>
+#include <memory>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <algorithm>
+
+#include "sg_internal.h"
+#include "sg_sim.h"
+
+static thread_local std::string g_err;
+void sg_set_error(const std::string &msg) { g_err = msg; }
+extern "C" const char *sg_last_error(void) { return g_err.c_str(); }
+extern "C" uint64_t sg_kernel_launches(void) { return sgk_launch_count(); }
+
+namespace {
+
+void destroy_impl(sg_sim *h)
+{
+    if (!h) return;
+    cudaStreamSynchronize(sgx_stream());
+    for (void *p : h->owned) sgx_free(p);
+    delete h;
+}
+
+int create_vb(sg_sim *h)
+{
+    cudaStream_t st = sgx_stream();
+    if (!sg_build_vb_graph(h->N, h->c, h->seed, h->g)) return SG_EINVAL;
+    VBHostGraph &g = h->g;
+    h->M = g.M;
+    const uint64_t N = h->N, W = h->W;
+    const uint64_t entries = g.col.size();
+    const uint64_t nslices = g.slice_ptr.size() - 1;
+    h->spin_words = N * W;
+    h->vb.spin = dev_alloc<uint64_t>(h, N * W);
+    h->vb.J = dev_alloc<uint64_t>(h, entries * W + 1);
+    h->vb.col = dev_alloc<uint32_t>(h, entries + 1);
+    h->vb.orig = dev_alloc<uint32_t>(h, N);
+    h->vb.deg = dev_alloc<uint8_t>(h, N);
+    h->vb.slice_ptr = dev_alloc<uint32_t>(h, nslices + 1);
+    h->vb.thr = dev_alloc<uint64_t>(h, 33);
+    uint32_t *eid_dev = dev_alloc<uint32_t>(h, entries + 1);
+    if (!h->vb.spin || !h->vb.J || !h->vb.col || !h->vb.orig || !h->vb.deg || !h->vb.slice_ptr || !h->vb.thr || !eid_dev)
+        return SG_ENOMEM;
+    h->thr_host = sg_vb_thresholds(h->T, g.dmax);
+    std::vector<uint64_t> thr33(33, 0);
+    for (size_t k = 0; k < h->thr_host.size() && k < 33; ++k) thr33[k] = h->thr_host[k];
+    if (!upload(h->vb.col, g.col, st) || !upload(h->vb.orig, g.orig, st) || !upload(h->vb.deg, g.deg, st) ||
+        !upload(h->vb.slice_ptr, g.slice_ptr, st) || !upload(h->vb.thr, thr33, st) || !upload(eid_dev, g.eid, st))
+        return SG_ECUDA;
+    int rc = sgk_init_vb_couplings(h->vb.J, eid_dev, entries, h->W, h->key, st);
+    if (rc) return rc;
+    rc = sgk_init_spins(h->vb.spin, h->vb.orig, N, h->W, h->key, st);
+    if (rc) return rc;
+    if (!cuda_ok(cudaStreamSynchronize(st), "sg_create")) return SG_ECUDA;
+    // the entry->edge table is only needed to draw the couplings; col/eid host copies are large: drop them
+    sgx_free(eid_dev);
+    h->owned.erase(std::find(h->owned.begin(), h->owned.end(), (void *)eid_dev));
+    std::vector<uint32_t>().swap(g.eid);
+    std::vector<uint32_t>().swap(g.col);
+    return SG_OK;
+}
+
+}  // namespace
+
+extern "C" sg_sim *sg_create(int model, uint64_t N, double c, double T, uint64_t seed, uint32_t n_words)
+{
+    g_err.clear();
+    if (model != SG_MODEL_VB && model != SG_MODEL_SK) { sg_set_error("sg_create: unknown model"); return nullptr; }
+    if (N < 2 || N >= (1ull << 32)) { sg_set_error("sg_create: N must satisfy 2 <= N < 2^32"); return nullptr; }
+    if (n_words == 0) { sg_set_error("sg_create: n_words must be >= 1"); return nullptr; }
+    if (!(T >= 0.0)) { sg_set_error("sg_create: T must be >= 0 (T = inf allowed)"); return nullptr; }
+    if (model == SG_MODEL_SK && N > 32768) { sg_set_error("sg_create: SK needs N <= 32768 (int16 local fields)"); return nullptr; }
+    std::string why;
+    if (!sgx_device_ok(&why)) { sg_set_error("sg_create: " + why); return nullptr; }
+    sg_sim *h = new (std::nothrow) sg_sim();
+    if (!h) { sg_set_error("sg_create: out of host memory"); return nullptr; }
+    h->model = model; h->N = N; h->W = n_words; h->c = c; h->T = T; h->seed = seed;
+    h->key = SGSeed{(uint32_t)seed, (uint32_t)(seed >> 32)};
+    int rc;
+    try {
+        rc = (model == SG_MODEL_VB) ? create_vb(h) : sg_sk_create_impl(h);
+        if (rc == SG_OK) {
+            h->counts_dev = dev_alloc<uint64_t>(h, 64ull * n_words);
+            if (!h->counts_dev) rc = SG_ENOMEM;
+        }
+    } catch (const std::bad_alloc &) {
+        sg_set_error("sg_create: out of host memory");
+        rc = SG_ENOMEM;
+    }
+    if (rc != SG_OK) { destroy_impl(h); return nullptr; }
+    return h;
+}
+
+extern "C" void sg_destroy(sg_sim *h) { destroy_impl(h); }
+
+extern "C" int sg_sweep(sg_sim *h, uint64_t n)
+{
+    if (!h) { sg_set_error("sg_sweep: null handle"); return SG_EINVAL; }
+    if (h->sweep + n >= (1ull << 56)) { sg_set_error("sg_sweep: sweep counter would exceed 2^56"); return SG_EINVAL; }
+    if (h->model == SG_MODEL_SK) return sg_sk_sweep_impl(h, n);
+    cudaStream_t st = sgx_stream();
+    for (uint64_t it = 0; it < n; ++it) {
+        for (uint32_t k = 0; k < h->g.K; ++k) {
+            const int rc = sgk_vb_sweep_class(h->vb, h->g.cls[k], h->W, h->sweep, h->key, st);
+            if (rc) return rc;
+        }
+        h->sweep++;
+    }
+    return SG_OK;
+}
+
+static uint64_t *current_config(sg_sim *h) { return h->model == SG_MODEL_VB ? h->vb.spin : h->sk.spin; }
+
+extern "C" int sg_snapshot(sg_sim *h, uint32_t slot)
+{
+    if (!h) { sg_set_error("sg_snapshot: null handle"); return SG_EINVAL; }
+    if (slot >= SG_MAX_SLOTS) { sg_set_error("sg_snapshot: slot out of range"); return SG_EINVAL; }
+    if (!h->slot[slot]) {
+        h->slot[slot] = dev_alloc<uint64_t>(h, h->spin_words);
+        if (!h->slot[slot]) return SG_ENOMEM;
+    }
+    if (!cuda_ok(cudaMemcpyAsync(h->slot[slot], current_config(h), h->spin_words * 8, cudaMemcpyDeviceToDevice, sgx_stream()),
+                 "sg_snapshot"))
+        return SG_ECUDA;
+    return SG_OK;
+}
+
+extern "C" int sg_correlation(sg_sim *h, uint32_t slot, uint64_t *out_counts)
+{
+    if (!h || !out_counts) { sg_set_error("sg_correlation: null argument"); return SG_EINVAL; }
+    if (slot >= SG_MAX_SLOTS) { sg_set_error("sg_correlation: slot out of range"); return SG_EINVAL; }
+    if (!h->slot[slot]) { sg_set_error("sg_correlation: slot was never written"); return SG_ESLOT; }
+    cudaStream_t st = sgx_stream();
+    const uint64_t lanes = 64ull * h->W;
+    if (!cuda_ok(cudaMemsetAsync(h->counts_dev, 0, lanes * 8, st), "sg_correlation")) return SG_ECUDA;
+    // Both layouts are site-major word-minor arrays of N*W words (VB: position order, the same
+    // permutation in both operands; SK: original order), so one kernel serves both models.
+    const int rc = sgk_xor_popcount(current_config(h), h->slot[slot], h->N, h->W, h->counts_dev, st);
+    if (rc) return rc;
+    if (!cuda_ok(cudaMemcpyAsync(out_counts, h->counts_dev, lanes * 8, cudaMemcpyDeviceToHost, st), "sg_correlation") ||
+        !cuda_ok(cudaStreamSynchronize(st), "sg_correlation"))
+        return SG_ECUDA;
+    return SG_OK;
+}
+
+extern "C" int sg_energy(sg_sim *h, int64_t *out)
+{
+    if (!h || !out) { sg_set_error("sg_energy: null argument"); return SG_EINVAL; }
+    if (h->model == SG_MODEL_SK) return sg_sk_energy_impl(h, out);
+    cudaStream_t st = sgx_stream();
+    const uint64_t lanes = 64ull * h->W;
+    if (!cuda_ok(cudaMemsetAsync(h->counts_dev, 0, lanes * 8, st), "sg_energy")) return SG_ECUDA;
+    for (uint32_t k = 0; k < h->g.K; ++k) {
+        const int rc = sgk_vb_unsat_class(h->vb, h->g.cls[k], h->W, h->counts_dev, st);
+        if (rc) return rc;
+    }
+    std::vector<uint64_t> twoU(lanes);
+    if (!cuda_ok(cudaMemcpyAsync(twoU.data(), h->counts_dev, lanes * 8, cudaMemcpyDeviceToHost, st), "sg_energy") ||
+        !cuda_ok(cudaStreamSynchronize(st), "sg_energy"))
+        return SG_ECUDA;
+    // sum_i u_i counts every unsatisfied bond from both ends: = 2U.  E = -(M - U) + U = 2U - M.
+    for (uint64_t l = 0; l < lanes; ++l) out[l] = (int64_t)twoU[l] - (int64_t)h->M;
+    return SG_OK;
+}
+
+// ---- getters ------------------------------------------------------------------------------------
+extern "C" uint64_t sg_sweep_count(const sg_sim *h) { return h ? h->sweep : 0; }
+extern "C" uint64_t sg_num_edges(const sg_sim *h) { return h ? h->M : 0; }
+extern "C" uint32_t sg_num_colours(const sg_sim *h) { return (h && h->model == SG_MODEL_VB) ? h->g.K : 0; }
+extern "C" uint32_t sg_max_degree(const sg_sim *h)
+{
+    if (!h) return 0;
+    return h->model == SG_MODEL_VB ? h->g.dmax : (uint32_t)(h->N - 1);
+}
+
+static bool ensure_scratch(sg_sim *h)
+{
+    if (!h->scratch) h->scratch = dev_alloc<uint64_t>(h, h->spin_words);
+    return h->scratch != nullptr;
+}
+
+extern "C" int sg_get_spins(sg_sim *h, int32_t slot, uint64_t *out)
+{
+    if (!h || !out) { sg_set_error("sg_get_spins: null argument"); return SG_EINVAL; }
+    const uint64_t *src = current_config(h);
+    if (slot >= 0) {
+        if (slot >= SG_MAX_SLOTS) { sg_set_error("sg_get_spins: slot out of range"); return SG_EINVAL; }
+        if (!h->slot[slot]) { sg_set_error("sg_get_spins: slot was never written"); return SG_ESLOT; }
+        src = h->slot[slot];
+    }
+    cudaStream_t st = sgx_stream();
+    if (h->model == SG_MODEL_SK) return sg_sk_get_spins_impl(h, src, out);
+    if (!ensure_scratch(h)) return SG_ENOMEM;
+    const int rc = sgk_permute_words(src, h->scratch, h->vb.orig, h->N, h->W, /*scatter=*/true, st);
+    if (rc) return rc;
+    if (!cuda_ok(cudaMemcpyAsync(out, h->scratch, h->N * h->W * 8, cudaMemcpyDeviceToHost, st), "sg_get_spins") ||
+        !cuda_ok(cudaStreamSynchronize(st), "sg_get_spins"))
+        return SG_ECUDA;
+    return SG_OK;
+}
+
+extern "C" int sg_set_spins(sg_sim *h, const uint64_t *in)
+{
+    if (!h || !in) { sg_set_error("sg_set_spins: null argument"); return SG_EINVAL; }
+    if (h->model == SG_MODEL_SK) return sg_sk_set_spins_impl(h, in);
+    cudaStream_t st = sgx_stream();
+    if (!ensure_scratch(h)) return SG_ENOMEM;
+    if (!cuda_ok(cudaMemcpyAsync(h->scratch, in, h->N * h->W * 8, cudaMemcpyHostToDevice, st), "sg_set_spins")) return SG_ECUDA;
+    const int rc = sgk_permute_words(h->scratch, h->vb.spin, h->vb.orig, h->N, h->W, /*scatter=*/false, st);
+    if (rc) return rc;
+    if (!cuda_ok(cudaStreamSynchronize(st), "sg_set_spins")) return SG_ECUDA;
+    return SG_OK;
+}
+
+extern "C" int sg_set_sweep_count(sg_sim *h, uint64_t t)
+{
+    if (!h || t >= (1ull << 56)) { sg_set_error("sg_set_sweep_count: bad argument"); return SG_EINVAL; }
+    h->sweep = t;
+    return SG_OK;
+}
+
+extern "C" int sg_get_graph(sg_sim *h, uint64_t *row_ptr, uint32_t *col, uint32_t *colour)
+{
+    if (!h || h->model != SG_MODEL_VB) { sg_set_error("sg_get_graph: VB handle required"); return SG_EINVAL; }
+    const VBHostGraph &g = h->g;
+    if (row_ptr) std::memcpy(row_ptr, g.row_ptr.data(), (g.N + 1) * sizeof(uint64_t));
+    if (col) std::memcpy(col, g.adj.data(), 2 * g.M * sizeof(uint32_t));
+    if (colour) for (uint64_t i = 0; i < g.N; ++i) colour[i] = g.colour[i];
+    return SG_OK;
+}
+
+extern "C" int sg_get_edges(sg_sim *h, uint32_t *u, uint32_t *v)
+{
+    if (!h || h->model != SG_MODEL_VB || !u || !v) { sg_set_error("sg_get_edges: VB handle required"); return SG_EINVAL; }
+    std::memcpy(u, h->g.eu.data(), h->g.M * sizeof(uint32_t));
+    std::memcpy(v, h->g.ev.data(), h->g.M * sizeof(uint32_t));
+    return SG_OK;
+}
+
+extern "C" int sg_get_couplings(sg_sim *h, uint64_t *out)
+{
+    if (!h || !out) { sg_set_error("sg_get_couplings: null argument"); return SG_EINVAL; }
+    if (h->model == SG_MODEL_SK) return sg_sk_get_couplings_impl(h, out);
+    cudaStream_t st = sgx_stream();
+    const uint64_t entries = 32ull * h->g.slice_ptr.back();
+    std::vector<uint64_t> J(entries * h->W);
+    if (!cuda_ok(cudaMemcpyAsync(J.data(), h->vb.J, J.size() * 8, cudaMemcpyDeviceToHost, st), "sg_get_couplings") ||
+        !cuda_ok(cudaStreamSynchronize(st), "sg_get_couplings"))
+        return SG_ECUDA;
+    const uint32_t W = h->W;
+    for (uint64_t e = 0; e < h->g.M; ++e) {
+        const uint64_t ent = h->g.entry_of_edge[e];
+        const uint64_t col32 = ent / 32, j = ent % 32;
+        for (uint32_t w = 0; w < W; ++w) out[e * W + w] = J[(col32 * 32) * W + j * W + w];
+    }
+    return SG_OK;
+}
+
+extern "C" int sg_get_thresholds(sg_sim *h, uint64_t *out, uint64_t n)
+{
+    if (!h || !out) { sg_set_error("sg_get_thresholds: null argument"); return SG_EINVAL; }
+    for (uint64_t k = 0; k < n; ++k) out[k] = k < h->thr_host.size() ? h->thr_host[k] : 0;
+    return SG_OK;
+}

@@ -1,0 +1,74 @@
+// sg_device.cuh -- device helpers: Philox4x32-10 (O1) and cache-hinted loads/stores.
+#pragma once
+#include <cstdint>
+
+// Philox4x32-10: 10 rounds of
+//   (c0,c1,c2,c3) <- (hi(B*c2)^c1^k0, lo(B*c2), hi(A*c0)^c3^k1, lo(A*c0)),  A=0xD2511F53, B=0xCD9E8D57
+// with (k0,k1) += (0x9E3779B9, 0xBB67AE85) between rounds.
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1, uint32_t (&out)[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t ha = __umulhi(0xD2511F53u, c0), la = 0xD2511F53u * c0;
+        const uint32_t hb = __umulhi(0xCD9E8D57u, c2), lb = 0xCD9E8D57u * c2;
+        c0 = hb ^ c1 ^ k0;
+        c2 = ha ^ c3 ^ k1;
+        c1 = lb;
+        c3 = la;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// L2 eviction policies.  The spin array is gathered at random (8 useful bytes per 32-byte sector)
+// and is re-read four times per sweep, so it is kept in L2 (evict_last); couplings, indices and
+// per-site metadata are touched once per sweep and stream through (evict_first, no L1 allocation).
+__device__ __forceinline__ uint64_t policy_evict_first()
+{
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t policy_evict_last()
+{
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t ld_stream_u64(const uint64_t *ptr, uint64_t pol)
+{
+    uint64_t v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.b64 %0, [%1], %2;" : "=l"(v) : "l"(ptr), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ uint32_t ld_stream_u32(const uint32_t *ptr, uint64_t pol)
+{
+    uint32_t v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.b32 %0, [%1], %2;" : "=r"(v) : "l"(ptr), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ uint32_t ld_stream_u8(const uint8_t *ptr, uint64_t pol)
+{
+    uint32_t v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.u8 %0, [%1], %2;" : "=r"(v) : "l"(ptr), "l"(pol));
+    return v;
+}
+// spin words: written by other classes' launches, so no .nc; keep in L2
+__device__ __forceinline__ uint64_t ld_keep_u64(const uint64_t *ptr, uint64_t pol)
+{
+    uint64_t v;
+    asm volatile("ld.global.L1::no_allocate.L2::cache_hint.b64 %0, [%1], %2;" : "=l"(v) : "l"(ptr), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ void st_keep_u64(uint64_t *ptr, uint64_t v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.b64 [%0], %1, %2;" ::"l"(ptr), "l"(v), "l"(pol) : "memory");
+}
+__device__ __forceinline__ uint64_t ld_plain_u64(const uint64_t *ptr)
+{
+    uint64_t v;
+    asm volatile("ld.global.b64 %0, [%1];" : "=l"(v) : "l"(ptr));
+    return v;
+}

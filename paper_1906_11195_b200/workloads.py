@@ -1,0 +1,78 @@
+"""BASELINE.json's configurations as parameter tuples, and the tw,t = 2^k measurement schedule.
+
+Shared by tests/ and bench.py (and by the oracle-side harness): it holds NO arithmetic of the
+method -- only which (model, N, c, T, seed, n_words, sweeps) to run and at which sweep counts to
+snapshot / correlate (O10).  Every instance is synthetic and follows from these
+parameters through the seeded generator each side implements for itself.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+
+VB, SK = 0, 1
+
+
+@dataclass(frozen=True)
+class Workload:
+    name: str
+    model: int
+    N: int
+    c: float
+    T: float
+    seed: int
+    n_words: int
+    sweeps: int
+
+
+# BASELINE.json configs[0..3]
+CFG1 = Workload("cfg1_vb_n1024", VB, 1 << 10, 4.0, 1.0, 1, 1, 1 << 10)
+CFG2 = Workload("cfg2_vb_n2^20_w4", VB, 1 << 20, 4.0, 1.0, 1, 4, 1 << 14)
+CFG3 = [Workload(f"cfg3_vb_n2^24_T{T}", VB, 1 << 24, 4.0, T, 1, 1, 1 << 12) for T in (0.6, 1.0, 1.4)]
+CFG4 = Workload("cfg4_sk_n4096", SK, 1 << 12, 0.0, 0.6, 1, 1, 1 << 12)
+
+
+def cfg5():
+    """BASELINE.json configs[4]: the aging protocol sweep (Q17/Q18)."""
+    out = []
+    for log2n, w, sweeps in ((12, 16, 1 << 16), (16, 16, 1 << 16), (20, 4, 1 << 16), (24, 1, 1 << 12), (26, 1, 1 << 12)):
+        for ti, T in enumerate((0.6, 1.0, 1.4)):
+            out.append(Workload(f"cfg5_vb_n2^{log2n}_T{T}", VB, 1 << log2n, 4.0, T, 1000 * log2n + ti, w, sweeps))
+    return out
+
+
+def schedule(total_sweeps: int):
+    """Events of the tw,t = 2^k protocol in time order (O10).
+
+    Yields (time, kind, slot) with kind 'snap' (slot a <- s(2^a)) or 'corr' (count against slot a at
+    time 2^a + 2^b).  Snapshots sort before correlations at equal times.
+    """
+    ev = []
+    a = 0
+    while (1 << a) <= total_sweeps:
+        ev.append((1 << a, 0, a))
+        b = 0
+        while (1 << a) + (1 << b) <= total_sweeps:
+            ev.append(((1 << a) + (1 << b), 1, a))
+            b += 1
+        a += 1
+    ev.sort()
+    return [(t, "snap" if k == 0 else "corr", s) for (t, k, s) in ev]
+
+
+def run_schedule(sim, total_sweeps: int):
+    """Drive any object with sweep/snapshot/correlation (the binding's Sim or the oracle's handle).
+
+    Returns {(tw, t): counts array}."""
+    out = {}
+    now = 0
+    for time, kind, slot in schedule(total_sweeps):
+        if time > now:
+            sim.sweep(time - now)
+            now = time
+        if kind == "snap":
+            sim.snapshot(slot)
+        else:
+            out[(1 << slot, time - (1 << slot))] = sim.correlation(slot).copy()
+    if now < total_sweeps:
+        sim.sweep(total_sweeps - now)
+    return out

@@ -1,0 +1,181 @@
+"""GPU parity (Viana-Bray): the CUDA path through the C-ABI vs the oracle, bit for bit.
+
+All integer work: spins, energies and correlation counts must be EQUAL (BASELINE.json north_star).
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def sg():
+    import torch
+
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1906_11195_b200 import build as b
+
+    b.build()
+    import paper_1906_11195_b200 as sg
+
+    return sg
+
+
+def _pair(sg, oracle_mod, N, c, T, seed, W):
+    g = sg.Sim(sg.SG_MODEL_VB, N, c, T, seed, W)
+    o = oracle_mod.Oracle(oracle_mod.VB, N, c, T, seed, W)
+    return g, o
+
+
+def _assert_same_state(g, o):
+    gs, os_ = g.spins(), o.spins()
+    if not np.array_equal(gs, os_):
+        bad = np.argwhere(gs != os_)
+        raise AssertionError(f"spins differ at {len(bad)} (site, word) places, first {bad[:5].tolist()}")
+    assert g.sweep_count == o.sweep_count
+
+
+@pytest.mark.parametrize("N,c,T,seed,W", [
+    (1024, 4.0, 1.0, 1, 1),      # config 1's instance
+    (1000, 4.0, 0.6, 2, 2),      # ragged sizes, W=2
+    (33, 3.0, 1.4, 3, 1),        # barely more than one slice
+    (4097, 4.0, 1.0, 4, 4),      # W=4 (32-byte site records)
+    (700, 6.0, 1.0, 5, 3),       # W not a power of two, higher degree
+    (2, 1.0, 1.0, 6, 1),         # two sites, one edge
+    (300, 0.0, 1.0, 7, 1),       # no edges: every site flips every sweep
+    (512, 12.0, 2.0, 8, 1),      # dense: degrees up to ~25, several chunks of 4 neighbours
+    (640, 4.0, 1.0, 9, 16),      # W=16 (config 5's small sizes)
+])
+def test_instance_and_first_sweeps_match(sg, oracle_mod, N, c, T, seed, W):
+    g, o = _pair(sg, oracle_mod, N, c, T, seed, W)
+    assert g.M == o.M and g.n_colours == o.n_colours and g.max_degree == o.max_degree
+    assert np.array_equal(g.edges(), o.edges())
+    grp, gcol, gcolour = g.graph()
+    orp, ocol, ocolour = o.graph()
+    assert np.array_equal(grp, orp) and np.array_equal(gcol, ocol) and np.array_equal(gcolour, ocolour)
+    assert np.array_equal(g.couplings(), o.couplings())
+    assert np.array_equal(g.thresholds(g.max_degree + 1), o.thresholds(o.max_degree + 1))
+    _assert_same_state(g, o)
+    assert np.array_equal(g.energy(), o.energy())
+    for _ in range(6):
+        g.sweep(1)
+        o.sweep(1)
+        _assert_same_state(g, o)
+        assert np.array_equal(g.energy(), o.energy())
+    g.sweep(5)
+    o.sweep(5)
+    _assert_same_state(g, o)
+
+
+def test_config1_full_protocol(sg, oracle_mod):
+    """BASELINE.json configs[0]: N=1024, 1024 sweeps, every sweep compared, all 100 (tw,t) pairs."""
+    from paper_1906_11195_b200.workloads import CFG1, run_schedule, schedule
+
+    w = CFG1
+    g = sg.Sim(w.model, w.N, w.c, w.T, w.seed, w.n_words)
+    o = oracle_mod.Oracle(w.model, w.N, w.c, w.T, w.seed, w.n_words)
+    g.snapshot(63)
+    assert np.all(g.correlation(63) == 0)                     # D = 0 at t = 0
+    events = {}
+    for t, kind, slot in schedule(w.sweeps):
+        events.setdefault(t, []).append((kind, slot))
+    ncorr = 0
+    for t in range(1, w.sweeps + 1):
+        g.sweep(1)
+        o.sweep(1)
+        assert np.array_equal(g.spins(), o.spins()), f"sweep {t}"
+        for kind, slot in events.get(t, []):
+            if kind == "snap":
+                g.snapshot(slot)
+                o.snapshot(slot)
+                assert np.all(g.correlation(slot) == 0)       # C(tw,tw) = 1
+            else:
+                assert np.array_equal(g.correlation(slot), o.correlation(slot)), (t, slot)
+                ncorr += 1
+        if t % 64 == 0:
+            assert np.array_equal(g.energy(), o.energy())
+    assert ncorr == 100
+    # and the same through the schedule driver in big sg_sweep(n) steps
+    g2 = sg.Sim(w.model, w.N, w.c, w.T, w.seed, w.n_words)
+    o2 = oracle_mod.Oracle(w.model, w.N, w.c, w.T, w.seed, w.n_words)
+    cg, co = run_schedule(g2, w.sweeps), run_schedule(o2, w.sweeps)
+    assert cg.keys() == co.keys() and len(cg) == 100
+    for k in cg:
+        assert np.array_equal(cg[k], co[k]), k
+    assert np.array_equal(g2.spins(), g.spins())
+
+
+@pytest.mark.parametrize("T", [0.0, float("inf"), 0.6, 1.4])
+def test_temperature_limits(sg, oracle_mod, T):
+    g, o = _pair(sg, oracle_mod, 3000, 4.0, T, 11, 1)
+    E0 = g.energy()
+    g.snapshot(0)
+    Eprev = E0
+    for t in range(1, 9):
+        g.sweep(1)
+        o.sweep(1)
+        _assert_same_state(g, o)
+        E = g.energy()
+        assert np.all((E - g.M) % 2 == 0)
+        if T == 0.0:
+            assert np.all(E <= Eprev)
+        if math.isinf(T):
+            assert np.array_equal(E, E0)
+            assert np.all(g.correlation(0) == (g.N if t % 2 else 0))
+        Eprev = E
+
+
+def test_sweep_is_a_pure_function_of_state_and_index(sg, oracle_mod):
+    """F_t spot check at a late sweep index, above 2^32 (uses the high counter word)."""
+    N, W = 5000, 2
+    g, o = _pair(sg, oracle_mod, N, 4.0, 1.0, 13, W)
+    rng = np.random.default_rng(5)
+    state = rng.integers(0, 1 << 64, size=(N, W), dtype=np.uint64)
+    for t in (4095, (1 << 32) - 1, (1 << 32) + 5, (1 << 55) + 123):
+        for h in (g, o):
+            h.set_spins(state)
+            h.set_sweep_count(t)
+            h.sweep(2)
+        _assert_same_state(g, o)
+
+
+def test_composition_and_slots(sg, oracle_mod):
+    a = sg.Sim(sg.SG_MODEL_VB, 2048, 4.0, 1.0, 21, 1)
+    b = sg.Sim(sg.SG_MODEL_VB, 2048, 4.0, 1.0, 21, 1)
+    a.sweep(3); a.sweep(0); a.sweep(4)
+    b.sweep(7)
+    assert np.array_equal(a.spins(), b.spins())
+    with pytest.raises(sg.SGError) as e:
+        a.correlation(5)
+    assert e.value.code == -4                                  # SG_ESLOT
+    with pytest.raises(sg.SGError):
+        a.snapshot(64)
+    a.snapshot(5)
+    assert np.array_equal(a.spins(5), a.spins())
+    a.sweep(1)
+    D = a.correlation(5)
+    from tests import exact
+    assert np.array_equal(D, (exact.unpack(a.spins(5)) != exact.unpack(a.spins())).sum(axis=0))
+
+
+@pytest.mark.parametrize("N,W,sweeps", [(1 << 16, 1, 24), (1 << 16, 4, 6), (1 << 18, 1, 5)])
+def test_mid_sizes_against_oracle(sg, oracle_mod, N, W, sweeps):
+    g, o = _pair(sg, oracle_mod, N, 4.0, 1.0, 1, W)
+    g.snapshot(0); o.snapshot(0)
+    for _ in range(sweeps // 3):
+        g.sweep(3)
+        o.sweep(3)
+        _assert_same_state(g, o)
+        assert np.array_equal(g.energy(), o.energy())
+        assert np.array_equal(g.correlation(0), o.correlation(0))
+
+
+def test_word_independence(sg):
+    """Q16: words share only graph and colouring; word w of a W=4 run is reproduced inside a W=8 run."""
+    a = sg.Sim(sg.SG_MODEL_VB, 3000, 4.0, 1.0, 5, 4)
+    b = sg.Sim(sg.SG_MODEL_VB, 3000, 4.0, 1.0, 5, 8)
+    a.sweep(5); b.sweep(5)
+    assert np.array_equal(a.spins(), b.spins()[:, :4])
+    assert np.array_equal(a.energy(), b.energy()[:256])

@@ -1,0 +1,138 @@
+"""CPU tests of the product's host side: the C-ABI library loads and exports every symbol of
+include/sg.h; its host Philox and host generator agree with the oracle; the device layout is
+self-consistent; without a GPU the compute calls fail loudly (no CPU fallback)."""
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def sg():
+    from paper_1906_11195_b200 import build as b
+
+    b.build()
+    import paper_1906_11195_b200 as sg
+
+    return sg
+
+
+def test_library_exports_every_declared_symbol(sg):
+    from paper_1906_11195_b200 import binding
+
+    L = sg.load_library()
+    hdr = open(os.path.join(ROOT, "include", "sg.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(sg_[a-z_0-9]+)\s*\(", hdr))
+    assert {"sg_create", "sg_sweep", "sg_snapshot", "sg_correlation", "sg_energy", "sg_destroy"} <= declared
+    for name in declared:
+        assert hasattr(L, name), name
+    assert declared == set(binding.SYMBOLS), declared ^ set(binding.SYMBOLS)
+
+
+def test_no_cpu_fallback(sg):
+    import torch
+
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(sg.SGError) as e:
+        sg.Sim(sg.SG_MODEL_VB, 1024, 4.0, 1.0, 1, 1)
+    assert "no CUDA device" in str(e.value) or "CUDA" in str(e.value)
+
+
+def test_bad_arguments_are_rejected_before_touching_the_gpu(sg):
+    for args in [(7, 100, 4.0, 1.0, 1, 1), (0, 1, 4.0, 1.0, 1, 1), (0, 100, 4.0, 1.0, 1, 0),
+                 (0, 100, 4.0, -0.5, 1, 1), (0, 100, 4.0, float("nan"), 1, 1), (1, 40000, 0.0, 1.0, 1, 1),
+                 (0, 1 << 32, 4.0, 1.0, 1, 1)]:
+        with pytest.raises(sg.SGError):
+            sg.Sim(*args)
+
+
+def test_host_philox_known_answers(sg):
+    from paper_1906_11195_b200 import binding
+
+    for line in open(os.path.join(ROOT, "tests", "golden", "philox_kat.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        v = [int(x, 16) for x in line.split()]
+        assert list(binding.host_philox(*v[:6])) == v[6:]
+
+
+@pytest.mark.parametrize("N,c,seed", [(1024, 4.0, 1), (5000, 4.0, 77), (333, 2.5, 3), (64, 7.0, 5), (100, 0.0, 1)])
+def test_host_generator_matches_oracle_and_layout_is_consistent(sg, oracle_mod, N, c, seed):
+    from paper_1906_11195_b200 import binding
+
+    g = binding.host_graph(N, c, seed)
+    o = oracle_mod.Oracle(oracle_mod.VB, N, c, 1.0, seed, 1)
+    assert g["M"] == o.M and g["K"] == o.n_colours and g["dmax"] == o.max_degree
+    e = o.edges()
+    assert np.array_equal(g["u"], e[:, 0]) and np.array_equal(g["v"], e[:, 1])
+    _, _, colour = o.graph()
+    assert np.array_equal(g["colour"], colour)
+    # positions: a permutation sorted by (colour, degree, label)
+    orig = g["orig"].astype(np.int64)
+    assert np.array_equal(np.sort(orig), np.arange(N))
+    degree = np.bincount(e.ravel().astype(np.int64), minlength=N)
+    key = list(zip(colour[orig].tolist(), degree[orig].tolist(), orig.tolist()))
+    assert key == sorted(key)
+    assert np.array_equal(g["deg"], degree[orig])
+    pos = np.empty(N, dtype=np.int64)
+    pos[orig] = np.arange(N)
+    # classes are contiguous position ranges; slices of 32; rows = neighbours in position space
+    nbrs = [set() for _ in range(N)]
+    for a, b in e.astype(np.int64):
+        nbrs[pos[a]].add(pos[b]); nbrs[pos[b]].add(pos[a])
+    sp = g["slice_ptr"].astype(np.int64)
+    seen_edges = np.zeros(g["M"], dtype=np.int64)
+    for k in range(g["K"]):
+        p0, n, s0 = int(g["class_pos0"][k]), int(g["class_n"][k]), int(g["class_slice0"][k])
+        assert np.all(colour[orig[p0:p0 + n]] == k)
+        for s in range((n + 31) // 32):
+            gs = s0 + s
+            D = sp[gs + 1] - sp[gs]
+            for j in range(32):
+                local = 32 * s + j
+                ents = 32 * sp[gs] + 32 * np.arange(D) + j
+                if local >= n:
+                    assert np.all(g["eid"][ents] == 0xFFFFFFFF)
+                    continue
+                p = p0 + local
+                d = int(g["deg"][p])
+                assert D >= d
+                assert set(g["col"][ents[:d]].tolist()) == nbrs[p] and len(nbrs[p]) == d
+                assert np.all(g["col"][ents[d:]] == p) and np.all(g["eid"][ents[d:]] == 0xFFFFFFFF)
+                for q in range(d):
+                    ed = int(g["eid"][ents[q]])
+                    a, b = int(e[ed, 0]), int(e[ed, 1])
+                    assert {pos[a], pos[b]} == {p, int(g["col"][ents[q]])}
+                    seen_edges[ed] += 1
+    assert np.all(seen_edges == 2)                      # every edge stored at both endpoints
+    assert g["entries"] == 32 * sp[-1]
+    # no edge inside a colour class (the race-freedom condition of the parallel update)
+    assert np.all(colour[e[:, 0]] != colour[e[:, 1]])
+
+
+def test_padding_overhead_is_small(sg):
+    from paper_1906_11195_b200 import binding
+
+    g = binding.host_graph(1 << 16, 4.0, 1)
+    assert g["entries"] <= 1.01 * 2 * g["M"]
+
+
+def test_schedule_counts():
+    from paper_1906_11195_b200.workloads import schedule
+
+    ev = schedule(1024)
+    assert sum(1 for x in ev if x[1] == "snap") == 11
+    assert sum(1 for x in ev if x[1] == "corr") == 100        # 100 pairs at config 1
+    assert all(ev[i][0] <= ev[i + 1][0] for i in range(len(ev) - 1))
+    snapped = set()
+    for t, kind, slot in ev:
+        if kind == "snap":
+            assert t == 1 << slot
+            snapped.add(slot)
+        else:
+            assert slot in snapped and t > (1 << slot) and bin(t - (1 << slot)).count("1") == 1
