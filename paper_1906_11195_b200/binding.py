@@ -89,6 +89,10 @@ def _ptr(a: np.ndarray):
 
 # ---- the five calls, C names --------------------------------------------------------------------
 def sg_create(model: int, N: int, c: float, T: float, seed: int, n_words: int) -> int:
+    import torch
+
+    if torch.cuda.is_available():
+        torch.cuda.init()   # the library takes memory from torch's caching allocator and its current stream
     h = load_library().sg_create(int(model), int(N), float(c), float(T), int(seed), int(n_words))
     if not h:
         raise SGError(SG_EINVAL, _err())

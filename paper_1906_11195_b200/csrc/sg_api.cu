@@ -141,8 +141,8 @@ extern "C" int sg_correlation(sg_sim *h, uint32_t slot, uint64_t *out_counts)
     cudaStream_t st = sgx_stream();
     const uint64_t lanes = 64ull * h->W;
     if (!cuda_ok(cudaMemsetAsync(h->counts_dev, 0, lanes * 8, st), "sg_correlation")) return SG_ECUDA;
-    // Both layouts are site-major word-minor arrays of N*W words (VB: position order, the same
-    // permutation in both operands; SK: original order), so one kernel serves both models.
+    if (h->model == SG_MODEL_SK) return sg_sk_correlation_impl(h, h->slot[slot], out_counts);
+    // position order in both operands (the same permutation), so no relabelling is needed
     const int rc = sgk_xor_popcount(current_config(h), h->slot[slot], h->N, h->W, h->counts_dev, st);
     if (rc) return rc;
     if (!cuda_ok(cudaMemcpyAsync(out_counts, h->counts_dev, lanes * 8, cudaMemcpyDeviceToHost, st), "sg_correlation") ||

@@ -56,6 +56,7 @@ bool upload(T *dst, const std::vector<T> &src, cudaStream_t st)
 int sg_sk_create_impl(sg_sim *h);
 int sg_sk_sweep_impl(sg_sim *h, uint64_t n);
 int sg_sk_energy_impl(sg_sim *h, int64_t *out);
+int sg_sk_correlation_impl(sg_sim *h, const uint64_t *slot_dev, uint64_t *out);
 int sg_sk_get_spins_impl(sg_sim *h, const uint64_t *src_dev, uint64_t *out);
 int sg_sk_set_spins_impl(sg_sim *h, const uint64_t *in);
 int sg_sk_get_couplings_impl(sg_sim *h, uint64_t *out);

@@ -12,6 +12,10 @@ void *sgx_alloc(size_t bytes)
 {
     if (bytes == 0) bytes = 8;
     try {
+        if (!c10::cuda::CUDACachingAllocator::get()->initialized()) {
+            sg_set_error("torch's CUDA allocator is not initialised: call torch.cuda.init() before sg_create");
+            return nullptr;
+        }
         return c10::cuda::CUDACachingAllocator::raw_alloc(bytes);
     } catch (const std::exception &e) {
         sg_set_error(std::string("device allocation of ") + std::to_string(bytes) + " bytes failed: " + e.what());
