@@ -1,0 +1,274 @@
+#!/usr/bin/env python
+"""bench.py -- spin updates/s of the Viana-Bray hot path on B200 (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--T 1.0]
+
+Workload (N=1): BASELINE.json configs[2], the bandwidth-bound roofline config: VB N=2^24, c=4, 64 samples
+(1 word) per site, T=1.0, seed 1.  One STEP = one pass of the whole hot path on the resident instance:
+  sg_sweep(SWEEPS_PER_STEP) + sg_snapshot + sg_correlation + sg_energy
+value = spin updates (Metropolis trials, Q23) of all ranks / device time (max over ranks).
+N>1: the path shards by sample: every rank runs its own 64-sample replica of the same
+recipe with seed+rank, no data-path collective ("weak" scaling).
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+SWEEPS_PER_STEP = 64
+BYTES_PER_SITE_WORD = 80.0          # own word 8 + 4 neighbour words 32 + 4 coupling words 32 + write-back 8
+CPU_SAMPLE_LOG2N = 22               # oracle sample: same recipe at N = 2^22
+METRIC = "spin updates/sec on 1 B200 (VB N=2^24, c=4) and % of HBM roofline"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=8)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--T", type=float, default=1.0)
+    ap.add_argument("--log2n", type=int, default=24)
+    ap.add_argument("--n-words", type=int, default=1)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+        sm = sorted(int(float(r[0])) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit())
+        mx = [int(float(r[1])) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for q, n in enumerate(names) if any(len(r) >= 7 and r[3 + q].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def dist_setup(n):
+    """One process per GPU; RANK/LOCAL_RANK/WORLD_SIZE/MASTER_* come from torchrun."""
+    rank, world, local = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1)), int(os.environ.get("LOCAL_RANK", 0))
+    return rank, world, local
+
+
+def cpu_sample(args, sweeps):
+    """Time the oracle, as it stands, on one host core: same recipe at N = 2^CPU_SAMPLE_LOG2N."""
+    import oracle
+
+    n = 1 << min(CPU_SAMPLE_LOG2N, args.log2n)
+    o = oracle.Oracle(oracle.VB, n, 4.0, args.T, 1, args.n_words)
+    t0 = time.perf_counter()
+    o.sweep(sweeps)
+    dt = time.perf_counter() - t0
+    return n * 64 * args.n_words * sweeps / dt, dt, n
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores; each step = 1 sweep of the N=2^22 sample."""
+    rank, world, _ = dist_setup(args.gpus)
+    if rank != 0:
+        return
+    import oracle
+
+    n = 1 << min(CPU_SAMPLE_LOG2N, args.log2n)
+    o = oracle.Oracle(oracle.VB, n, 4.0, args.T, 1, args.n_words)
+    for _ in range(args.warmup):
+        o.sweep(1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.sweep(1)
+    dt = time.perf_counter() - t0
+    val = n * 64 * args.n_words * args.steps / dt
+    sample = f"VB c=4 T={args.T} seed 1, same recipe at N=2^{n.bit_length() - 1} (bounded sample), 1 oracle sweep per step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "spin updates/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+        "config": {"workload": f"VB N=2^{args.log2n} c=4 W={args.n_words} T={args.T} seed=1 (BASELINE.json configs[2])", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": "spin updates/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "spin updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    rank, world, local = dist_setup(args.gpus)
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_1906_11195_b200 import build as b
+
+    if rank == 0:
+        b.build()
+    if world > 1:
+        dist.barrier()
+    import paper_1906_11195_b200 as sg
+
+    N, W = 1 << args.log2n, args.n_words
+    t0 = time.perf_counter()
+    sim = sg.Sim(sg.SG_MODEL_VB, N, 4.0, args.T, 1 + rank, W)
+    create_s = time.perf_counter() - t0
+    counts = np.zeros(64 * W, dtype=np.uint64)
+    energy = np.zeros(64 * W, dtype=np.int64)
+    sweep_ev = []
+
+    def step(timed):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        sim.sweep(SWEEPS_PER_STEP)
+        e1.record()
+        sim.snapshot(0)
+        sim.correlation(0, counts)
+        sim.energy(energy)
+        if timed:
+            sweep_ev.append((e0, e1))
+
+    def sync_all():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step(False)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = sg.kernel_launches()
+    sync_all()
+    s_ev, f_ev = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    s_ev.record()
+    for _ in range(args.steps):
+        step(True)
+    f_ev.record()
+    sync_all()
+    launches = sg.kernel_launches() - l0
+    clocks = sampler.stop() if rank == 0 else None
+    ms = s_ev.elapsed_time(f_ev)
+    sweep_ms = sum(a.elapsed_time(b_) for a, b_ in sweep_ev)
+    if world > 1:
+        t = torch.tensor([ms, sweep_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, sweep_ms = float(t[0]), float(t[1])
+    updates_per_rank = N * 64 * W * SWEEPS_PER_STEP * args.steps
+    value = updates_per_rank * world / (ms * 1e-3)
+
+    # ---- e2e: the same step through the C-ABI with HOST buffers: the configuration goes in from pinned host
+    # memory (sg_set_spins) and comes back (sg_get_spins) every step, as in the paper's flow
+    e2e = None
+    if not args.no_e2e:
+        host = torch.empty((N, W), dtype=torch.int64, pin_memory=True).numpy().view(np.uint64)
+        sim.spins(out=host)
+        for _ in range(2):
+            sim.set_spins(host); step(False); sim.spins(out=host)
+        sync_all()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            sim.set_spins(host)
+            step(False)
+            sim.spins(out=host)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t[0])
+        e2e = {"value": updates_per_rank * world / dt, "unit": "spin updates/s",
+               "h2d_bytes_per_step": N * W * 8, "d2h_bytes_per_step": N * W * 8 + 2 * 64 * W * 8,
+               "note": "sg_set_spins(pinned host) + step + sg_get_spins(pinned host) per step, wall clock"}
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    peak, peak_src = peaks()
+    site_words = N * W * SWEEPS_PER_STEP * args.steps
+    achieved = BYTES_PER_SITE_WORD * site_words / (sweep_ms * 1e-3) / 1e9
+    out = {
+        "metric": METRIC, "value": value, "unit": "spin updates/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+        "config": {"workload": f"VB N=2^{args.log2n} c=4 W={W} T={args.T} seed=1+rank (BASELINE.json configs[2])",
+                   "step": f"sg_sweep({SWEEPS_PER_STEP}) + sg_snapshot + sg_correlation + sg_energy",
+                   "l2": "inputs larger than L2 (couplings+indices 768 MiB, spins 128 MiB streamed every sweep)",
+                   "parallelism": "replicas sharded by sample word, no data-path collective" if world > 1 else "single GPU",
+                   "create_s": round(create_s, 2)},
+        "roofline": {"bound": "hbm", "kernel": "k_vb_sweep (all colour classes of a sweep)", "achieved": achieved, "peak": peak,
+                     "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                     "bytes_per_site_word": BYTES_PER_SITE_WORD, "sweep_ms": sweep_ms / (SWEEPS_PER_STEP * args.steps),
+                     "sweep_share_of_step": sweep_ms / ms},
+        "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+    }
+    tr = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tr):
+        out["roofline"]["traffic"] = json.load(open(tr)).get("dram_bytes_per_sweep")
+    if not args.no_cpu_baseline:
+        v, dt, n = cpu_sample(args, 2)
+        out["cpu_baseline"] = {"value": v, "unit": "spin updates/s", "cores": 1, "kind": "oracle", "host_cores": os.cpu_count(),
+                               "sample": f"same recipe at N=2^{n.bit_length() - 1}, 2 oracle sweeps, {dt:.1f} s"}
+    out["context"] = {"paper": "~15 ps per spin update on one P100 = 6.7e10 spin updates/s (PAPER.md:320); "
+                               "total work of the order of 2^64 spin updates (PAPER.md:165)"}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

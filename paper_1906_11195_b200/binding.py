@@ -184,8 +184,10 @@ class Sim:
     def max_degree(self) -> int:
         return self._L.sg_max_degree(self._h)
 
-    def spins(self, slot: int = -1) -> np.ndarray:
-        out = np.zeros((self.N, self.W), dtype=np.uint64)
+    def spins(self, slot: int = -1, out: np.ndarray | None = None) -> np.ndarray:
+        if out is None:
+            out = np.zeros((self.N, self.W), dtype=np.uint64)
+        assert out.dtype == np.uint64 and out.flags.c_contiguous and out.size == self.N * self.W
         _check(self._L.sg_get_spins(self._h, slot, _ptr(out)))
         return out
 
