@@ -42,6 +42,7 @@ def parse():
     ap.add_argument("--n-words", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--sweeps-per-step", type=int, default=SWEEPS_PER_STEP)
     return ap.parse_args()
 
 
@@ -263,7 +264,9 @@ def run_ours(args):
 
 
 def main():
+    global SWEEPS_PER_STEP
     args = parse()
+    SWEEPS_PER_STEP = args.sweeps_per_step
     if args.impl == "reference":
         run_reference(args)
     else:
