@@ -40,7 +40,7 @@ enum { SG_OK = 0, SG_EINVAL = -1, SG_ENOMEM = -2, SG_ECUDA = -3, SG_ESLOT = -4 }
  *                        M = floor(c*N/2 + 0.5), self-loops and multi-edges rejected (O2);
  *           SG_MODEL_SK: Sherrington-Kirkpatrick model (Eq. 1) with binary couplings
  *                        +-1/sqrt(N); c is ignored.
- *   N       number of sites, 2 <= N < 2^32 (SK: N <= 32768 so that int16 local fields are exact).
+ *   N       number of sites, 2 <= N < 2^31 (SK: N <= 32768 so that int16 local fields are exact).
  *   c       mean degree (VB), c >= 0 and M <= N(N-1)/2.
  *   T       temperature, 0 <= T <= +inf (T = 0 and T = inf are legal).
  *   seed    Philox key.  (model, N, c, T, seed, n_words) determine every bit of every output.
@@ -134,24 +134,27 @@ void sg_host_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t
 
 /*
  * The VB instance exactly as sg_create lays it out for the device, built on
- * the host only.  Sites are relabelled to positions p sorted by (colour, degree, label); a colour class
- * is cut into slices of 32 positions; slice g stores its rows column-major: entry 32*slice_ptr[g] + 32*k + j
- * is the k-th neighbour (a position) of the j-th site of the slice; padding entries hold the site's own
- * position and edge id 0xFFFFFFFF.
+ * the host only.  Sites are relabelled to positions p sorted by (colour, degree, label); every
+ * (colour, degree) bucket starts at a multiple of 32, the gap positions being padding (orig = 0xFFFFFFFF).
+ * Slice g = positions 32g .. 32g+31 holds sites of one degree D = slice_ptr[g+1] - slice_ptr[g] and stores
+ * its rows column-major: entry 32*slice_ptr[g] + 32*k + j is the k-th neighbour (a position) of the j-th
+ * site of the slice; padding positions point at themselves with edge id 0xFFFFFFFF.  A tile (2 uint64:
+ * first neighbour column | first position << 32, then nslices in bits 0-3 and the row lengths in 5-bit
+ * fields from bit 4) groups up to 8 consecutive slices of one class for the staged sweep kernel.
  */
 typedef struct sg_host_graph sg_host_graph;
 sg_host_graph *sg_host_graph_create(uint64_t N, double c, uint64_t seed);   /* NULL on bad arguments */
 void sg_host_graph_destroy(sg_host_graph *g);
-/* info HOST 6 uint64: M, K (colours), dmax, entries, nslices, N */
+/* info HOST 8 uint64: M, K (colours), dmax, entries, nslices, N, P (positions incl. padding), ntiles */
 int sg_host_graph_info(const sg_host_graph *g, uint64_t *info);
 /*
- * Copies out whichever arrays are non-NULL (all HOST): u,v M uint32; colour N uint32; orig N uint32
- * (position -> label); deg N uint32 (per position); slice_ptr nslices+1 uint32; col entries uint32;
- * eid entries uint32; class_pos0, class_n, class_slice0 K uint64 each.
+ * Copies out whichever arrays are non-NULL (all HOST): u,v M uint32; colour N uint32; orig P uint32
+ * (position -> label); deg P uint32 (per position); slice_ptr nslices+1 uint32; col entries uint32;
+ * eid entries uint32; class_pos0, class_n, class_slice0 K uint64 each; tiles 2*ntiles uint64.
  */
 int sg_host_graph_get(const sg_host_graph *g, uint32_t *u, uint32_t *v, uint32_t *colour, uint32_t *orig,
                       uint32_t *deg, uint32_t *slice_ptr, uint32_t *col, uint32_t *eid,
-                      uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0);
+                      uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0, uint64_t *tiles);
 
 /*
  * Number of kernels this library has launched (process-wide, all handles) since load.

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <memory>
 #include <new>
@@ -35,29 +36,49 @@ int create_vb(sg_sim *h)
     if (!sg_build_vb_graph(h->N, h->c, h->seed, h->g)) return SG_EINVAL;
     VBHostGraph &g = h->g;
     h->M = g.M;
-    const uint64_t N = h->N, W = h->W;
+    const uint64_t N = h->N, W = h->W, P = g.P;
     const uint64_t entries = g.col.size();
     const uint64_t nslices = g.slice_ptr.size() - 1;
-    h->spin_words = N * W;
-    h->vb.spin = dev_alloc<uint64_t>(h, N * W);
+    h->spin_words = P * W;
+    h->vb.spin = dev_alloc<uint64_t>(h, P * W);
     h->vb.J = dev_alloc<uint64_t>(h, entries * W + 1);
     h->vb.col = dev_alloc<uint32_t>(h, entries + 1);
-    h->vb.orig = dev_alloc<uint32_t>(h, N);
-    h->vb.deg = dev_alloc<uint8_t>(h, N);
+    h->vb.orig = dev_alloc<uint32_t>(h, P);
+    h->vb.tiles = dev_alloc<VBTile>(h, g.tiles.size() + 1);
     h->vb.slice_ptr = dev_alloc<uint32_t>(h, nslices + 1);
     h->vb.thr = dev_alloc<uint64_t>(h, 33);
     uint32_t *eid_dev = dev_alloc<uint32_t>(h, entries + 1);
-    if (!h->vb.spin || !h->vb.J || !h->vb.col || !h->vb.orig || !h->vb.deg || !h->vb.slice_ptr || !h->vb.thr || !eid_dev)
+    if (!h->vb.spin || !h->vb.J || !h->vb.col || !h->vb.orig || !h->vb.tiles || !h->vb.slice_ptr || !h->vb.thr || !eid_dev)
         return SG_ENOMEM;
+    // Hot set: the spins of sites with degree >= dhot are kept in L2 (they are gathered d times per sweep).
+    // Budget in MiB (SG_HOT_MB, default 48): the largest high-degree set whose spin words fit.
+    {
+        double budget_mb = 48.0;
+        if (const char *e = std::getenv("SG_HOT_MB")) budget_mb = std::atof(e);
+        std::vector<uint64_t> hist(g.dmax + 2, 0);
+        for (uint64_t p = 0; p < P; ++p) hist[g.deg[p]]++;   // padding counted: it occupies the array too
+        uint32_t dhot = g.dmax + 1;
+        uint64_t sites = 0;
+        while (dhot > 0 && (double)(sites + hist[dhot - 1]) * 8.0 * (double)W <= budget_mb * 1048576.0) sites += hist[--dhot];
+        h->vb.dhot = dhot;
+        for (uint64_t q = 0; q < entries; ++q)
+            if (g.deg[g.col[q]] >= dhot) g.col[q] |= 0x80000000u;
+    }
+    h->vb_fast = sgk_vb_sweep_fast_ok(P, entries, h->W);
+    h->vb_staged = sgk_vb_sweep_staged_ok(P, entries, h->W);
+    if (const char *e = std::getenv("SG_VB_KERNEL")) {      // experiments: force a simpler kernel
+        if (!std::strcmp(e, "fast")) h->vb_staged = false;
+        if (!std::strcmp(e, "general")) h->vb_staged = h->vb_fast = false;
+    }
     h->thr_host = sg_vb_thresholds(h->T, g.dmax);
     std::vector<uint64_t> thr33(33, 0);
     for (size_t k = 0; k < h->thr_host.size() && k < 33; ++k) thr33[k] = h->thr_host[k];
-    if (!upload(h->vb.col, g.col, st) || !upload(h->vb.orig, g.orig, st) || !upload(h->vb.deg, g.deg, st) ||
+    if (!upload(h->vb.col, g.col, st) || !upload(h->vb.orig, g.orig, st) || !upload(h->vb.tiles, g.tiles, st) ||
         !upload(h->vb.slice_ptr, g.slice_ptr, st) || !upload(h->vb.thr, thr33, st) || !upload(eid_dev, g.eid, st))
         return SG_ECUDA;
     int rc = sgk_init_vb_couplings(h->vb.J, eid_dev, entries, h->W, h->key, st);
     if (rc) return rc;
-    rc = sgk_init_spins(h->vb.spin, h->vb.orig, N, h->W, h->key, st);
+    rc = sgk_init_spins(h->vb.spin, h->vb.orig, P, h->W, h->key, st);
     if (rc) return rc;
     if (!cuda_ok(cudaStreamSynchronize(st), "sg_create")) return SG_ECUDA;
     // the entry->edge table is only needed to draw the couplings; col/eid host copies are large: drop them
@@ -74,7 +95,7 @@ extern "C" sg_sim *sg_create(int model, uint64_t N, double c, double T, uint64_t
 {
     g_err.clear();
     if (model != SG_MODEL_VB && model != SG_MODEL_SK) { sg_set_error("sg_create: unknown model"); return nullptr; }
-    if (N < 2 || N >= (1ull << 32)) { sg_set_error("sg_create: N must satisfy 2 <= N < 2^32"); return nullptr; }
+    if (N < 2 || N >= (1ull << 31)) { sg_set_error("sg_create: N must satisfy 2 <= N < 2^31"); return nullptr; }
     if (n_words == 0) { sg_set_error("sg_create: n_words must be >= 1"); return nullptr; }
     if (!(T >= 0.0)) { sg_set_error("sg_create: T must be >= 0 (T = inf allowed)"); return nullptr; }
     if (model == SG_MODEL_SK && N > 32768) { sg_set_error("sg_create: SK needs N <= 32768 (int16 local fields)"); return nullptr; }
@@ -109,7 +130,9 @@ extern "C" int sg_sweep(sg_sim *h, uint64_t n)
     cudaStream_t st = sgx_stream();
     for (uint64_t it = 0; it < n; ++it) {
         for (uint32_t k = 0; k < h->g.K; ++k) {
-            const int rc = sgk_vb_sweep_class(h->vb, h->g.cls[k], h->W, h->sweep, h->key, st);
+            const int rc = h->vb_staged ? sgk_vb_sweep_class_staged(h->vb, h->g.cls[k], h->sweep, h->key, st)
+                           : h->vb_fast ? sgk_vb_sweep_class_fast(h->vb, h->g.cls[k], h->W, h->sweep, h->key, st)
+                                      : sgk_vb_sweep_class(h->vb, h->g.cls[k], h->W, h->sweep, h->key, st);
             if (rc) return rc;
         }
         h->sweep++;
@@ -143,7 +166,7 @@ extern "C" int sg_correlation(sg_sim *h, uint32_t slot, uint64_t *out_counts)
     if (!cuda_ok(cudaMemsetAsync(h->counts_dev, 0, lanes * 8, st), "sg_correlation")) return SG_ECUDA;
     if (h->model == SG_MODEL_SK) return sg_sk_correlation_impl(h, h->slot[slot], out_counts);
     // position order in both operands (the same permutation), so no relabelling is needed
-    const int rc = sgk_xor_popcount(current_config(h), h->slot[slot], h->N, h->W, h->counts_dev, st);
+    const int rc = sgk_xor_popcount(current_config(h), h->slot[slot], h->g.P, h->W, h->counts_dev, st);
     if (rc) return rc;
     if (!cuda_ok(cudaMemcpyAsync(out_counts, h->counts_dev, lanes * 8, cudaMemcpyDeviceToHost, st), "sg_correlation") ||
         !cuda_ok(cudaStreamSynchronize(st), "sg_correlation"))
@@ -183,7 +206,7 @@ extern "C" uint32_t sg_max_degree(const sg_sim *h)
 
 static bool ensure_scratch(sg_sim *h)
 {
-    if (!h->scratch) h->scratch = dev_alloc<uint64_t>(h, h->spin_words);
+    if (!h->scratch) h->scratch = dev_alloc<uint64_t>(h, h->N * h->W);   // original order, no padding
     return h->scratch != nullptr;
 }
 
@@ -199,7 +222,7 @@ extern "C" int sg_get_spins(sg_sim *h, int32_t slot, uint64_t *out)
     cudaStream_t st = sgx_stream();
     if (h->model == SG_MODEL_SK) return sg_sk_get_spins_impl(h, src, out);
     if (!ensure_scratch(h)) return SG_ENOMEM;
-    const int rc = sgk_permute_words(src, h->scratch, h->vb.orig, h->N, h->W, /*scatter=*/true, st);
+    const int rc = sgk_permute_words(src, h->scratch, h->vb.orig, h->g.P, h->W, /*scatter=*/true, st);
     if (rc) return rc;
     if (!cuda_ok(cudaMemcpyAsync(out, h->scratch, h->N * h->W * 8, cudaMemcpyDeviceToHost, st), "sg_get_spins") ||
         !cuda_ok(cudaStreamSynchronize(st), "sg_get_spins"))
@@ -214,7 +237,7 @@ extern "C" int sg_set_spins(sg_sim *h, const uint64_t *in)
     cudaStream_t st = sgx_stream();
     if (!ensure_scratch(h)) return SG_ENOMEM;
     if (!cuda_ok(cudaMemcpyAsync(h->scratch, in, h->N * h->W * 8, cudaMemcpyHostToDevice, st), "sg_set_spins")) return SG_ECUDA;
-    const int rc = sgk_permute_words(h->scratch, h->vb.spin, h->vb.orig, h->N, h->W, /*scatter=*/false, st);
+    const int rc = sgk_permute_words(h->scratch, h->vb.spin, h->vb.orig, h->g.P, h->W, /*scatter=*/false, st);
     if (rc) return rc;
     if (!cuda_ok(cudaStreamSynchronize(st), "sg_set_spins")) return SG_ECUDA;
     return SG_OK;

@@ -132,74 +132,87 @@ bool sg_build_vb_graph(uint64_t N, double c, uint64_t seed, VBHostGraph &g)
         K = std::max(K, col + 1);
     }
     g.K = K;
-    // positions: counting sort by (colour, degree), ties by original label
+    // Positions: sites sorted by (colour, degree, original label).  Every (colour, degree) bucket starts
+    // at a multiple of 32 positions; the gap positions are padding (orig = NONE, spin word 0, never
+    // written), so a slice of 32 positions holds sites of ONE degree: no padded neighbour slots, and the
+    // degree of a site is the slice's row length.
     const uint32_t DB = g.dmax + 1;
-    std::vector<uint64_t> bucket((uint64_t)K * DB + 1, 0);
-    for (uint64_t i = 0; i < N; ++i) {
-        const uint64_t d = g.row_ptr[i + 1] - g.row_ptr[i];
-        bucket[(uint64_t)g.colour[i] * DB + d + 1]++;
-    }
-    for (size_t b = 1; b < bucket.size(); ++b) bucket[b] += bucket[b - 1];
+    std::vector<uint64_t> cnt((uint64_t)K * DB, 0), start((uint64_t)K * DB + 1, 0);
+    for (uint64_t i = 0; i < N; ++i) cnt[(uint64_t)g.colour[i] * DB + (g.row_ptr[i + 1] - g.row_ptr[i])]++;
+    for (size_t b = 0; b < cnt.size(); ++b) start[b + 1] = start[b] + ((cnt[b] + 31) / 32) * 32;
+    const uint64_t P = start[cnt.size()];
+    if (P >= (1ull << 31)) { sg_set_error("sg_create: too many sites"); return false; }
+    g.P = P;
     g.cls.assign(K, VBClass{});
     for (uint32_t k = 0; k < K; ++k) {
-        g.cls[k].pos0 = bucket[(uint64_t)k * DB];
-        g.cls[k].n = bucket[(uint64_t)(k + 1) * DB] - bucket[(uint64_t)k * DB];
+        g.cls[k].pos0 = start[(uint64_t)k * DB];
+        g.cls[k].n = start[(uint64_t)(k + 1) * DB] - start[(uint64_t)k * DB];
     }
-    g.orig.resize(N); g.pos.resize(N); g.deg.resize(N);
-    for (uint64_t i = 0; i < N; ++i) {
-        const uint64_t d = g.row_ptr[i + 1] - g.row_ptr[i];
-        const uint64_t p = bucket[(uint64_t)g.colour[i] * DB + d]++;
-        g.orig[p] = (uint32_t)i; g.pos[i] = (uint32_t)p; g.deg[p] = (uint8_t)d;
-    }
-    // sliced ELL
-    uint64_t nslices = 0;
-    for (uint32_t k = 0; k < K; ++k) {
-        g.cls[k].slice0 = nslices;
-        g.cls[k].nslices = (g.cls[k].n + 31) / 32;
-        nslices += g.cls[k].nslices;
-    }
-    g.slice_ptr.assign(nslices + 1, 0);
+    g.orig.assign(P, SG_NONE); g.pos.resize(N); g.deg.assign(P, 0);
     for (uint32_t k = 0; k < K; ++k)
-        for (uint64_t s = 0; s < g.cls[k].nslices; ++s) {
-            const uint64_t pa = g.cls[k].pos0 + 32 * s;
-            const uint64_t pb = std::min(pa + 32, g.cls[k].pos0 + g.cls[k].n);
-            uint32_t D = 0;
-            for (uint64_t p = pa; p < pb; ++p) D = std::max<uint32_t>(D, g.deg[p]);
-            g.slice_ptr[g.cls[k].slice0 + s + 1] = D;
+        for (uint32_t d = 0; d < DB; ++d)
+            for (uint64_t p = start[(uint64_t)k * DB + d]; p < start[(uint64_t)k * DB + d + 1]; ++p) g.deg[p] = (uint8_t)d;
+    {
+        std::vector<uint64_t> fill(start.begin(), start.end() - 1);
+        for (uint64_t i = 0; i < N; ++i) {
+            const uint64_t p = fill[(uint64_t)g.colour[i] * DB + (g.row_ptr[i + 1] - g.row_ptr[i])]++;
+            g.orig[p] = (uint32_t)i; g.pos[i] = (uint32_t)p;
         }
+    }
+    // sliced ELL: slice s of the whole position space = positions 32 s .. 32 s + 31, row length deg[32 s]
+    const uint64_t nslices = P / 32;
+    g.slice_ptr.assign(nslices + 1, 0);
     for (uint64_t s = 0; s < nslices; ++s) {
-        const uint64_t next = (uint64_t)g.slice_ptr[s] + g.slice_ptr[s + 1];
+        const uint64_t next = (uint64_t)g.slice_ptr[s] + g.deg[32 * s];
         if (next > 0x7FFFFFFull) { sg_set_error("sg_create: instance too large for 32-bit entry indices"); return false; }
         g.slice_ptr[s + 1] = (uint32_t)next;
     }
+    for (uint32_t k = 0; k < K; ++k) { g.cls[k].slice0 = g.cls[k].pos0 / 32; g.cls[k].nslices = g.cls[k].n / 32; }
     const uint64_t entries = 32ull * g.slice_ptr[nslices];
-    g.col.resize(entries); g.eid.assign(entries, 0xFFFFFFFFu);
+    g.col.resize(entries); g.eid.assign(entries, SG_NONE);
     g.entry_of_edge.assign(M, 0);
-    for (uint32_t k = 0; k < K; ++k)
-        for (uint64_t s = 0; s < g.cls[k].nslices; ++s) {
-            const uint64_t gs = g.cls[k].slice0 + s;
-            const uint64_t base = 32ull * g.slice_ptr[gs];
-            const uint32_t D = g.slice_ptr[gs + 1] - g.slice_ptr[gs];
-            for (uint32_t j = 0; j < 32; ++j) {
-                const uint64_t local = 32 * s + j;
-                const bool valid = local < g.cls[k].n;
-                const uint64_t p = g.cls[k].pos0 + (valid ? local : 0);
-                const uint32_t i = g.orig[p];
-                const uint64_t r0 = g.row_ptr[i];
-                const uint32_t d = valid ? g.deg[p] : 0;
-                for (uint32_t q = 0; q < D; ++q) {
-                    const uint64_t ent = base + 32ull * q + j;
-                    if (q < d) {
-                        g.col[ent] = g.pos[g.adj[r0 + q]];
-                        const uint32_t e = g.adj_e[r0 + q];
-                        g.eid[ent] = e;
-                        if (g.eu[e] == i) g.entry_of_edge[e] = (uint32_t)ent;
-                    } else {
-                        g.col[ent] = (uint32_t)p;   // padding: own position, coupling word 0
-                    }
+    for (uint64_t s = 0; s < nslices; ++s) {
+        const uint64_t base = 32ull * g.slice_ptr[s];
+        const uint32_t D = g.slice_ptr[s + 1] - g.slice_ptr[s];
+        for (uint32_t j = 0; j < 32; ++j) {
+            const uint64_t p = 32 * s + j;
+            const uint32_t i = g.orig[p];
+            for (uint32_t q = 0; q < D; ++q) {
+                const uint64_t ent = base + 32ull * q + j;
+                if (i != SG_NONE) {
+                    const uint64_t r0 = g.row_ptr[i];
+                    g.col[ent] = g.pos[g.adj[r0 + q]];
+                    const uint32_t e = g.adj_e[r0 + q];
+                    g.eid[ent] = e;
+                    if (g.eu[e] == i) g.entry_of_edge[e] = (uint32_t)ent;
+                } else {
+                    g.col[ent] = (uint32_t)p;   // padding position: points at itself, coupling word 0
                 }
             }
         }
+    }
+    // tiles for the staged sweep kernel: consecutive slices of one class, at most SG_TILE_SLICES slices
+    // and SG_TILE_ENT32 neighbour columns (32 entries each)
+    g.tiles.clear();
+    for (uint32_t k = 0; k < K; ++k) {
+        g.cls[k].tile0 = g.tiles.size();
+        uint64_t s = g.cls[k].slice0;
+        const uint64_t send = s + g.cls[k].nslices;
+        while (s < send) {
+            VBTile t{g.slice_ptr[s], (uint32_t)(32 * s), 0};
+            uint32_t ns = 0, cols = 0;
+            while (s + ns < send && ns < SG_TILE_SLICES) {
+                const uint32_t D = g.slice_ptr[s + ns + 1] - g.slice_ptr[s + ns];
+                if (ns > 0 && cols + D > SG_TILE_ENT32) break;
+                t.packed |= (uint64_t)D << (4 + 5 * ns);
+                cols += D; ++ns;
+            }
+            t.packed |= ns;
+            g.tiles.push_back(t);
+            s += ns;
+        }
+        g.cls[k].ntiles = g.tiles.size() - g.cls[k].tile0;
+    }
     return true;
 }
 
@@ -226,13 +239,13 @@ extern "C" int sg_host_graph_info(const sg_host_graph *h, uint64_t *info)
 {
     if (!h || !info) return SG_EINVAL;
     info[0] = h->g.M; info[1] = h->g.K; info[2] = h->g.dmax; info[3] = h->g.col.size();
-    info[4] = h->g.slice_ptr.size() - 1; info[5] = h->g.N;
+    info[4] = h->g.slice_ptr.size() - 1; info[5] = h->g.N; info[6] = h->g.P; info[7] = h->g.tiles.size();
     return SG_OK;
 }
 
 extern "C" int sg_host_graph_get(const sg_host_graph *h, uint32_t *u, uint32_t *v, uint32_t *colour, uint32_t *orig,
                                  uint32_t *deg, uint32_t *slice_ptr, uint32_t *col, uint32_t *eid,
-                                 uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0)
+                                 uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0, uint64_t *tiles)
 {
     if (!h) return SG_EINVAL;
     const VBHostGraph &g = h->g;
@@ -249,5 +262,7 @@ extern "C" int sg_host_graph_get(const sg_host_graph *h, uint32_t *u, uint32_t *
         if (class_n) class_n[k] = g.cls[k].n;
         if (class_slice0) class_slice0[k] = g.cls[k].slice0;
     }
+    if (tiles) std::memcpy(tiles, g.tiles.data(), g.tiles.size() * sizeof(VBTile));
+    if (tiles) std::memcpy(tiles, g.tiles.data(), g.tiles.size() * sizeof(VBTile));
     return SG_OK;
 }

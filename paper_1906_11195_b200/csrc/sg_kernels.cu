@@ -24,7 +24,7 @@ void sgk_count_launch() { g_launches.fetch_add(1); }
     } while (0)
 
 // ------------------------------------------------------------------------------------ init
-// O4: sigma_p[w] = x0 | x1<<32 of P(orig[p], w, 0, tag 1)
+// O4: sigma_p[w] = x0 | x1<<32 of P(orig[p], w, 0, tag 1); N here = number of positions
 __global__ void __launch_bounds__(256) k_init_spins(uint64_t *__restrict__ spin, const uint32_t *__restrict__ orig,
                                                     uint64_t N, uint32_t W, uint32_t k0, uint32_t k1)
 {
@@ -33,6 +33,7 @@ __global__ void __launch_bounds__(256) k_init_spins(uint64_t *__restrict__ spin,
     const uint64_t p = q / W;
     const uint32_t w = (uint32_t)(q % W);
     const uint32_t site = orig ? orig[p] : (uint32_t)p;
+    if (site == SG_NONE) { spin[q] = 0; return; }   // padding position
     uint32_t x[4];
     philox4x32_10(site, w, 0u, 1u << 24, k0, k1, x);
     spin[q] = (uint64_t)x[0] | ((uint64_t)x[1] << 32);
@@ -112,8 +113,8 @@ __device__ __forceinline__ Planes5 count_unsatisfied(const uint64_t *__restrict_
         }
 #pragma unroll
         for (int q = 0; q < 4; ++q)
-            if (k + q < D) sn[q] = SPIN_HINT ? ld_keep_u64(spin + (uint64_t)nb[q] * W + w, pol_keep)
-                                     : ld_plain_u64(spin + (uint64_t)nb[q] * W + w);
+            if (k + q < D) sn[q] = SPIN_HINT ? ld_keep_u64(spin + (uint64_t)(nb[q] & 0x7FFFFFFFu) * W + w, pol_keep)
+                                     : ld_plain_u64(spin + (uint64_t)(nb[q] & 0x7FFFFFFFu) * W + w);
         uint64_t m[4];
 #pragma unroll
         for (int q = 0; q < 4; ++q) m[q] = (k + q < D) ? (own ^ sn[q] ^ jw[q]) : 0ull;
@@ -149,7 +150,7 @@ __device__ __forceinline__ uint64_t lanes_ge(const Planes5 &P, uint32_t umin)
 
 __global__ void __launch_bounds__(256)
 k_vb_sweep(uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, const uint32_t *__restrict__ col,
-           const uint32_t *__restrict__ orig, const uint8_t *__restrict__ deg, const uint32_t *__restrict__ slice_ptr,
+           const uint32_t *__restrict__ orig, const uint32_t *__restrict__ slice_ptr,
            const uint64_t *__restrict__ thr, uint64_t pos0, uint64_t n_sites, uint64_t slice0, uint64_t nslices,
            uint32_t W, uint32_t sweep_lo, uint32_t sweep_hi, uint32_t k0, uint32_t k1)
 {
@@ -169,8 +170,9 @@ k_vb_sweep(uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, const ui
     const uint32_t D = sp1 - sp0;
     uint64_t *own_ptr = spin + p * W + w;
     const uint64_t own = ld_keep_u64(own_ptr, pol_keep);
-    const uint32_t d = ld_stream_u8(deg + p, pol_stream);
+    const uint32_t d = D;   // slices hold sites of one degree
     const uint32_t site = ld_stream_u32(orig + p, pol_stream);
+    if (site == SG_NONE) return;   // padding position
 
     const Planes5 P = count_unsatisfied<true>(spin, J, col, 32ull * sp0, D, j, t, w, W, own, pol_stream, pol_keep);
 
@@ -192,7 +194,7 @@ int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint32_t W, uint64_t
     if (c.n == 0) return SG_OK;
     const uint64_t threads = c.nslices * 32ull * W;
     const unsigned grid = (unsigned)((threads + 255) / 256);
-    k_vb_sweep<<<grid, 256, 0, st>>>(d.spin, d.J, d.col, d.orig, d.deg, d.slice_ptr, d.thr, c.pos0, c.n, c.slice0,
+    k_vb_sweep<<<grid, 256, 0, st>>>(d.spin, d.J, d.col, d.orig, d.slice_ptr, d.thr, c.pos0, c.n, c.slice0,
                                      c.nslices, W, (uint32_t)sweep, (uint32_t)(sweep >> 32) /* tag 0 */, key.k0, key.k1);
     SG_LAUNCH_CHECK();
     return SG_OK;
@@ -392,6 +394,7 @@ int sgk_vb_unsat_class(const VBDevice &d, const VBClass &c, uint32_t W, uint64_t
 }
 
 // ------------------------------------------------------------------------------------ relabelling helper
+// N = number of positions (padding included); map = orig
 // scatter: dst[map[p]*W + w] = src[p*W + w]   (position order -> original order)
 // gather : dst[p*W + w] = src[map[p]*W + w]   (original order -> position order)
 __global__ void __launch_bounds__(256) k_permute_words(const uint64_t *__restrict__ src, uint64_t *__restrict__ dst,
@@ -401,7 +404,12 @@ __global__ void __launch_bounds__(256) k_permute_words(const uint64_t *__restric
     if (q >= N * W) return;
     const uint64_t p = q / W;
     const uint32_t w = (uint32_t)(q % W);
-    const uint64_t other = (uint64_t)map[p] * W + w;
+    const uint32_t m = map[p];
+    if (m == SG_NONE) {            // padding position: nothing to export, stays 0 on import
+        if (!scatter) dst[q] = 0;
+        return;
+    }
+    const uint64_t other = (uint64_t)m * W + w;
     if (scatter) dst[other] = src[q];
     else dst[q] = src[other];
 }

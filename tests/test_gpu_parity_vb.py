@@ -179,3 +179,17 @@ def test_word_independence(sg):
     a.sweep(5); b.sweep(5)
     assert np.array_equal(a.spins(), b.spins()[:, :4])
     assert np.array_equal(a.energy(), b.energy()[:256])
+
+
+@pytest.mark.parametrize("kernel", ["staged", "fast", "general"])
+@pytest.mark.parametrize("N,c,T,seed", [(1 << 14, 4.0, 1.0, 3), (5000, 9.0, 1.4, 4), (100, 4.0, 0.6, 5)])
+def test_every_sweep_kernel_variant_matches_oracle(sg, oracle_mod, monkeypatch, kernel, N, c, T, seed):
+    """n_words = 1 has three implementations of the sweep (persistent TMA-staged, thread-per-site,
+    general-W); SG_VB_KERNEL picks one at sg_create.  All must equal the oracle."""
+    monkeypatch.setenv("SG_VB_KERNEL", kernel)
+    g, o = _pair(sg, oracle_mod, N, c, T, seed, 1)
+    for _ in range(4):
+        g.sweep(2)
+        o.sweep(2)
+        _assert_same_state(g, o)
+    assert np.array_equal(g.energy(), o.energy())

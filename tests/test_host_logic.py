@@ -46,7 +46,7 @@ def test_no_cpu_fallback(sg):
 def test_bad_arguments_are_rejected_before_touching_the_gpu(sg):
     for args in [(7, 100, 4.0, 1.0, 1, 1), (0, 1, 4.0, 1.0, 1, 1), (0, 100, 4.0, 1.0, 1, 0),
                  (0, 100, 4.0, -0.5, 1, 1), (0, 100, 4.0, float("nan"), 1, 1), (1, 40000, 0.0, 1.0, 1, 1),
-                 (0, 1 << 32, 4.0, 1.0, 1, 1)]:
+                 (0, 1 << 31, 4.0, 1.0, 1, 1)]:
         with pytest.raises(sg.SGError):
             sg.Sim(*args)
 
@@ -72,54 +72,79 @@ def test_host_generator_matches_oracle_and_layout_is_consistent(sg, oracle_mod, 
     assert np.array_equal(g["u"], e[:, 0]) and np.array_equal(g["v"], e[:, 1])
     _, _, colour = o.graph()
     assert np.array_equal(g["colour"], colour)
-    # positions: a permutation sorted by (colour, degree, label)
-    orig = g["orig"].astype(np.int64)
+    # positions: valid positions are a permutation of the labels sorted by (colour, degree, label);
+    # every (colour, degree) bucket starts at a multiple of 32, gaps are padding (orig = NONE)
+    NONE = 0xFFFFFFFF
+    P = g["P"]
+    assert P % 32 == 0 and g["nslices"] == P // 32
+    orig_all = g["orig"].astype(np.int64)
+    valid = orig_all != NONE
+    orig = orig_all[valid]
     assert np.array_equal(np.sort(orig), np.arange(N))
     degree = np.bincount(e.ravel().astype(np.int64), minlength=N)
     key = list(zip(colour[orig].tolist(), degree[orig].tolist(), orig.tolist()))
     assert key == sorted(key)
-    assert np.array_equal(g["deg"], degree[orig])
+    assert np.array_equal(g["deg"][valid], degree[orig])
     pos = np.empty(N, dtype=np.int64)
-    pos[orig] = np.arange(N)
-    # classes are contiguous position ranges; slices of 32; rows = neighbours in position space
-    nbrs = [set() for _ in range(N)]
+    pos[orig] = np.nonzero(valid)[0]
+    sp = g["slice_ptr"].astype(np.int64)
+    # one degree per slice (padding carries its bucket's degree), and it is the slice's row length
+    degs = g["deg"].astype(np.int64).reshape(-1, 32)
+    assert np.all(degs == degs[:, :1]) and np.array_equal(np.diff(sp), degs[:, 0])
+    # padding never exceeds 31 positions per (colour, degree) bucket
+    assert P - N <= 31 * g["K"] * (g["dmax"] + 1)
+    nbrs = [set() for _ in range(P)]
     for a, b in e.astype(np.int64):
         nbrs[pos[a]].add(pos[b]); nbrs[pos[b]].add(pos[a])
-    sp = g["slice_ptr"].astype(np.int64)
     seen_edges = np.zeros(g["M"], dtype=np.int64)
     for k in range(g["K"]):
         p0, n, s0 = int(g["class_pos0"][k]), int(g["class_n"][k]), int(g["class_slice0"][k])
-        assert np.all(colour[orig[p0:p0 + n]] == k)
-        for s in range((n + 31) // 32):
-            gs = s0 + s
-            D = sp[gs + 1] - sp[gs]
-            for j in range(32):
-                local = 32 * s + j
-                ents = 32 * sp[gs] + 32 * np.arange(D) + j
-                if local >= n:
-                    assert np.all(g["eid"][ents] == 0xFFFFFFFF)
-                    continue
-                p = p0 + local
-                d = int(g["deg"][p])
-                assert D >= d
-                assert set(g["col"][ents[:d]].tolist()) == nbrs[p] and len(nbrs[p]) == d
-                assert np.all(g["col"][ents[d:]] == p) and np.all(g["eid"][ents[d:]] == 0xFFFFFFFF)
-                for q in range(d):
-                    ed = int(g["eid"][ents[q]])
-                    a, b = int(e[ed, 0]), int(e[ed, 1])
-                    assert {pos[a], pos[b]} == {p, int(g["col"][ents[q]])}
-                    seen_edges[ed] += 1
+        assert p0 % 32 == 0 and n % 32 == 0 and s0 == p0 // 32
+        cls_orig = orig_all[p0:p0 + n]
+        assert np.all(colour[cls_orig[cls_orig != NONE]] == k)
+    for s_ in range(P // 32):
+        D = sp[s_ + 1] - sp[s_]
+        for j in range(32):
+            p = 32 * s_ + j
+            ents = 32 * sp[s_] + 32 * np.arange(D) + j
+            if orig_all[p] == NONE:
+                assert np.all(g["eid"][ents] == NONE) and np.all(g["col"][ents] == p)
+                continue
+            assert set(g["col"][ents].tolist()) == nbrs[p] and len(nbrs[p]) == D
+            for q in range(D):
+                ed = int(g["eid"][ents[q]])
+                a, b = int(e[ed, 0]), int(e[ed, 1])
+                assert {pos[a], pos[b]} == {p, int(g["col"][ents[q]])}
+                seen_edges[ed] += 1
     assert np.all(seen_edges == 2)                      # every edge stored at both endpoints
     assert g["entries"] == 32 * sp[-1]
     # no edge inside a colour class (the race-freedom condition of the parallel update)
     assert np.all(colour[e[:, 0]] != colour[e[:, 1]])
+    # tiles: cover every class's slices once, in order, within the staging limits
+    tiles = g["tiles"]
+    nxt = {int(g["class_slice0"][k]): k for k in range(g["K"])}
+    s_expect = 0
+    for ent_pos, packed in tiles.tolist():
+        ent32, tpos0 = ent_pos & 0xFFFFFFFF, ent_pos >> 32
+        ns = packed & 15
+        assert 1 <= ns <= 8 and tpos0 == 32 * s_expect and ent32 == sp[s_expect]
+        Ds = [(packed >> (4 + 5 * q)) & 31 for q in range(ns)]
+        assert Ds == np.diff(sp[s_expect:s_expect + ns + 1]).tolist()
+        assert sum(Ds) <= 32 or ns == 1
+        k_of = [k for k in range(g["K"]) if int(g["class_slice0"][k]) <= s_expect < int(g["class_slice0"][k]) + int(g["class_n"][k]) // 32]
+        assert len(k_of) == 1 and s_expect + ns <= int(g["class_slice0"][k_of[0]]) + int(g["class_n"][k_of[0]]) // 32
+        s_expect += ns
+    assert s_expect == P // 32
 
 
 def test_padding_overhead_is_small(sg):
     from paper_1906_11195_b200 import binding
 
-    g = binding.host_graph(1 << 16, 4.0, 1)
-    assert g["entries"] <= 1.01 * 2 * g["M"]
+    g = binding.host_graph(1 << 18, 4.0, 1)
+    # at most 31 padding positions per (colour, degree) bucket: a constant, negligible at large N
+    assert g["entries"] <= 2 * g["M"] + 31 * g["K"] * sum(range(g["dmax"] + 1))
+    assert g["entries"] <= 1.02 * 2 * g["M"]
+    assert g["P"] <= 1.01 * g["N"]
 
 
 def test_schedule_counts():
