@@ -134,27 +134,29 @@ void sg_host_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t
 
 /*
  * The VB instance exactly as sg_create lays it out for the device, built on
- * the host only.  Sites are relabelled to positions p sorted by (colour, degree, label); every
- * (colour, degree) bucket starts at a multiple of 32, the gap positions being padding (orig = 0xFFFFFFFF).
- * Slice g = positions 32g .. 32g+31 holds sites of one degree D = slice_ptr[g+1] - slice_ptr[g] and stores
- * its rows column-major: entry 32*slice_ptr[g] + 32*k + j is the k-th neighbour (a position) of the j-th
- * site of the slice; padding positions point at themselves with edge id 0xFFFFFFFF.  A tile (2 uint64:
- * first neighbour column | first position << 32, then nslices in bits 0-3 and the row lengths in 5-bit
- * fields from bit 4) groups up to 8 consecutive slices of one class for the staged sweep kernel.
+ * the host only.  Sites are relabelled to positions p: class-major (colour 0, 1, ...), every class starting
+ * at a multiple of 32, the gap positions being padding (orig = 0xFFFFFFFF).  Inside a class the sites keep
+ * their breadth-first index order (BFS over the whole graph, roots in label order, rows in edge order): the
+ * locality-improving relabelling; every window of `sort_window` consecutive sites of a class is then stably
+ * sorted by degree.  Slice g = positions 32g .. 32g+31 has row length D = slice_ptr[g+1] - slice_ptr[g] = the
+ * largest degree in the slice and stores its rows column-major: entry 32*slice_ptr[g] + 32*k + j is the k-th
+ * neighbour (a position) of the j-th site of the slice.  Entries beyond a site's degree, and all entries of
+ * padding positions, point at the site's own position with edge id 0xFFFFFFFF (coupling word 0).
+ * No output depends on this relabelling: the Philox counter uses the original label (Q15).
  */
 typedef struct sg_host_graph sg_host_graph;
 sg_host_graph *sg_host_graph_create(uint64_t N, double c, uint64_t seed);   /* NULL on bad arguments */
 void sg_host_graph_destroy(sg_host_graph *g);
-/* info HOST 8 uint64: M, K (colours), dmax, entries, nslices, N, P (positions incl. padding), ntiles */
+/* info HOST 8 uint64: M, K (colours), dmax, entries, nslices, N, P (positions incl. padding), sort_window */
 int sg_host_graph_info(const sg_host_graph *g, uint64_t *info);
 /*
  * Copies out whichever arrays are non-NULL (all HOST): u,v M uint32; colour N uint32; orig P uint32
- * (position -> label); deg P uint32 (per position); slice_ptr nslices+1 uint32; col entries uint32;
- * eid entries uint32; class_pos0, class_n, class_slice0 K uint64 each; tiles 2*ntiles uint64.
+ * (position -> label); deg P uint32 (per position, 0 for padding); slice_ptr nslices+1 uint32; col entries
+ * uint32; eid entries uint32; class_pos0, class_n, class_slice0 K uint64 each.
  */
 int sg_host_graph_get(const sg_host_graph *g, uint32_t *u, uint32_t *v, uint32_t *colour, uint32_t *orig,
                       uint32_t *deg, uint32_t *slice_ptr, uint32_t *col, uint32_t *eid,
-                      uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0, uint64_t *tiles);
+                      uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0);
 
 /*
  * Number of kernels this library has launched (process-wide, all handles) since load.

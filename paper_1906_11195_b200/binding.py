@@ -42,7 +42,7 @@ SYMBOLS = {
     "sg_host_graph_create": (_vp, [_u64, _dbl, _u64]),
     "sg_host_graph_destroy": (None, [_vp]),
     "sg_host_graph_info": (C.c_int, [_vp, _vp]),
-    "sg_host_graph_get": (C.c_int, [_vp] * 13),
+    "sg_host_graph_get": (C.c_int, [_vp] * 12),
 }
 
 
@@ -238,8 +238,8 @@ def host_graph(N: int, c: float, seed: int) -> dict:
     try:
         info = np.zeros(8, dtype=np.uint64)
         _check(L.sg_host_graph_info(g, _ptr(info)))
-        M, K, dmax, entries, nslices, N, P, ntiles = (int(x) for x in info)
-        a = dict(M=M, K=K, dmax=dmax, entries=entries, nslices=nslices, N=N, P=P, ntiles=ntiles)
+        M, K, dmax, entries, nslices, N, P, sort_window = (int(x) for x in info)
+        a = dict(M=M, K=K, dmax=dmax, entries=entries, nslices=nslices, N=N, P=P, sort_window=sort_window)
         a["u"] = np.zeros(M, np.uint32); a["v"] = np.zeros(M, np.uint32)
         a["colour"] = np.zeros(N, np.uint32)
         for k in ("orig", "deg"):
@@ -248,10 +248,9 @@ def host_graph(N: int, c: float, seed: int) -> dict:
         a["col"] = np.zeros(entries, np.uint32); a["eid"] = np.zeros(entries, np.uint32)
         for k in ("class_pos0", "class_n", "class_slice0"):
             a[k] = np.zeros(K, np.uint64)
-        a["tiles"] = np.zeros((ntiles, 2), np.uint64)
         _check(L.sg_host_graph_get(g, _ptr(a["u"]), _ptr(a["v"]), _ptr(a["colour"]), _ptr(a["orig"]), _ptr(a["deg"]),
                                    _ptr(a["slice_ptr"]), _ptr(a["col"]), _ptr(a["eid"]), _ptr(a["class_pos0"]),
-                                   _ptr(a["class_n"]), _ptr(a["class_slice0"]), _ptr(a["tiles"])))
+                                   _ptr(a["class_n"]), _ptr(a["class_slice0"])))
         return a
     finally:
         L.sg_host_graph_destroy(g)

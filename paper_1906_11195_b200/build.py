@@ -12,7 +12,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsg.so")
 OBJ = os.path.join(HERE, "build")
 
-CU = ["sg_kernels.cu", "sg_vb_sweep.cu", "sg_vb_staged.cu", "sg_sk.cu", "sg_api.cu"]
+CU = ["sg_kernels.cu", "sg_vb_sweep.cu", "sg_sk.cu", "sg_api.cu"]
 CPP = ["sg_host.cpp", "sg_torch_glue.cpp"]
 
 

@@ -36,44 +36,24 @@ int create_vb(sg_sim *h)
     if (!sg_build_vb_graph(h->N, h->c, h->seed, h->g)) return SG_EINVAL;
     VBHostGraph &g = h->g;
     h->M = g.M;
-    const uint64_t N = h->N, W = h->W, P = g.P;
+    const uint64_t W = h->W, P = g.P;
     const uint64_t entries = g.col.size();
     const uint64_t nslices = g.slice_ptr.size() - 1;
     h->spin_words = P * W;
+    h->vb_entries = entries;
     h->vb.spin = dev_alloc<uint64_t>(h, P * W);
     h->vb.J = dev_alloc<uint64_t>(h, entries * W + 1);
     h->vb.col = dev_alloc<uint32_t>(h, entries + 1);
     h->vb.orig = dev_alloc<uint32_t>(h, P);
-    h->vb.tiles = dev_alloc<VBTile>(h, g.tiles.size() + 1);
     h->vb.slice_ptr = dev_alloc<uint32_t>(h, nslices + 1);
     h->vb.thr = dev_alloc<uint64_t>(h, 33);
     uint32_t *eid_dev = dev_alloc<uint32_t>(h, entries + 1);
-    if (!h->vb.spin || !h->vb.J || !h->vb.col || !h->vb.orig || !h->vb.tiles || !h->vb.slice_ptr || !h->vb.thr || !eid_dev)
+    if (!h->vb.spin || !h->vb.J || !h->vb.col || !h->vb.orig || !h->vb.slice_ptr || !h->vb.thr || !eid_dev)
         return SG_ENOMEM;
-    // Hot set: the spins of sites with degree >= dhot are kept in L2 (they are gathered d times per sweep).
-    // Budget in MiB (SG_HOT_MB, default 48): the largest high-degree set whose spin words fit.
-    {
-        double budget_mb = 48.0;
-        if (const char *e = std::getenv("SG_HOT_MB")) budget_mb = std::atof(e);
-        std::vector<uint64_t> hist(g.dmax + 2, 0);
-        for (uint64_t p = 0; p < P; ++p) hist[g.deg[p]]++;   // padding counted: it occupies the array too
-        uint32_t dhot = g.dmax + 1;
-        uint64_t sites = 0;
-        while (dhot > 0 && (double)(sites + hist[dhot - 1]) * 8.0 * (double)W <= budget_mb * 1048576.0) sites += hist[--dhot];
-        h->vb.dhot = dhot;
-        for (uint64_t q = 0; q < entries; ++q)
-            if (g.deg[g.col[q]] >= dhot) g.col[q] |= 0x80000000u;
-    }
-    h->vb_fast = sgk_vb_sweep_fast_ok(P, entries, h->W);
-    h->vb_staged = sgk_vb_sweep_staged_ok(P, entries, h->W);
-    if (const char *e = std::getenv("SG_VB_KERNEL")) {      // experiments: force a simpler kernel
-        if (!std::strcmp(e, "fast")) h->vb_staged = false;
-        if (!std::strcmp(e, "general")) h->vb_staged = h->vb_fast = false;
-    }
     h->thr_host = sg_vb_thresholds(h->T, g.dmax);
     std::vector<uint64_t> thr33(33, 0);
     for (size_t k = 0; k < h->thr_host.size() && k < 33; ++k) thr33[k] = h->thr_host[k];
-    if (!upload(h->vb.col, g.col, st) || !upload(h->vb.orig, g.orig, st) || !upload(h->vb.tiles, g.tiles, st) ||
+    if (!upload(h->vb.col, g.col, st) || !upload(h->vb.orig, g.orig, st) ||
         !upload(h->vb.slice_ptr, g.slice_ptr, st) || !upload(h->vb.thr, thr33, st) || !upload(eid_dev, g.eid, st))
         return SG_ECUDA;
     int rc = sgk_init_vb_couplings(h->vb.J, eid_dev, entries, h->W, h->key, st);
@@ -130,9 +110,7 @@ extern "C" int sg_sweep(sg_sim *h, uint64_t n)
     cudaStream_t st = sgx_stream();
     for (uint64_t it = 0; it < n; ++it) {
         for (uint32_t k = 0; k < h->g.K; ++k) {
-            const int rc = h->vb_staged ? sgk_vb_sweep_class_staged(h->vb, h->g.cls[k], h->sweep, h->key, st)
-                           : h->vb_fast ? sgk_vb_sweep_class_fast(h->vb, h->g.cls[k], h->W, h->sweep, h->key, st)
-                                      : sgk_vb_sweep_class(h->vb, h->g.cls[k], h->W, h->sweep, h->key, st);
+            const int rc = sgk_vb_sweep_class(h->vb, h->g.cls[k], h->g.P, h->vb_entries, h->W, h->sweep, h->key, st);
             if (rc) return rc;
         }
         h->sweep++;

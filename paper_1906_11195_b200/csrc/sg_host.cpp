@@ -3,6 +3,7 @@
 // Independent of oracle/: nothing here is shared with or derived from it.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <numeric>
 
@@ -132,38 +133,79 @@ bool sg_build_vb_graph(uint64_t N, double c, uint64_t seed, VBHostGraph &g)
         K = std::max(K, col + 1);
     }
     g.K = K;
-    // Positions: sites sorted by (colour, degree, original label).  Every (colour, degree) bucket starts
-    // at a multiple of 32 positions; the gap positions are padding (orig = NONE, spin word 0, never
-    // written), so a slice of 32 positions holds sites of ONE degree: no padded neighbour slots, and the
-    // degree of a site is the slice's row length.
-    const uint32_t DB = g.dmax + 1;
-    std::vector<uint64_t> cnt((uint64_t)K * DB, 0), start((uint64_t)K * DB + 1, 0);
-    for (uint64_t i = 0; i < N; ++i) cnt[(uint64_t)g.colour[i] * DB + (g.row_ptr[i + 1] - g.row_ptr[i])]++;
-    for (size_t b = 0; b < cnt.size(); ++b) start[b + 1] = start[b] + ((cnt[b] + 31) / 32) * 32;
-    const uint64_t P = start[cnt.size()];
-    if (P >= (1ull << 31)) { sg_set_error("sg_create: too many sites"); return false; }
-    g.P = P;
-    g.cls.assign(K, VBClass{});
-    for (uint32_t k = 0; k < K; ++k) {
-        g.cls[k].pos0 = start[(uint64_t)k * DB];
-        g.cls[k].n = start[(uint64_t)(k + 1) * DB] - start[(uint64_t)k * DB];
-    }
-    g.orig.assign(P, SG_NONE); g.pos.resize(N); g.deg.assign(P, 0);
-    for (uint32_t k = 0; k < K; ++k)
-        for (uint32_t d = 0; d < DB; ++d)
-            for (uint64_t p = start[(uint64_t)k * DB + d]; p < start[(uint64_t)k * DB + d + 1]; ++p) g.deg[p] = (uint8_t)d;
-    {
-        std::vector<uint64_t> fill(start.begin(), start.end() - 1);
-        for (uint64_t i = 0; i < N; ++i) {
-            const uint64_t p = fill[(uint64_t)g.colour[i] * DB + (g.row_ptr[i + 1] - g.row_ptr[i])]++;
-            g.orig[p] = (uint32_t)i; g.pos[i] = (uint32_t)p;
+    // Locality order (the "locality-improving relabelling within each colour class" of BASELINE.json): breadth-first
+    // index over the whole graph, roots in label order, rows in stored order.  The graph is locally tree-like, so
+    // a site's tree parent and children get nearby indices; since a class keeps this order, the gathers along the
+    // N-1 tree edges (half of all gathers at c = 4) walk through every other class's block monotonically and find
+    // their 32-byte sectors still in L2 (or L1) instead of costing a DRAM row activation each.
+    // (SG_VB_ORDER=label keeps the label order instead: a measurement knob, see profiles/; outputs are identical.)
+    std::vector<uint32_t> bfs; bfs.reserve(N);
+    const char *order_env = std::getenv("SG_VB_ORDER");
+    if (order_env && !std::strcmp(order_env, "label")) {
+        bfs.resize(N);
+        std::iota(bfs.begin(), bfs.end(), 0u);
+    } else {
+        std::vector<uint8_t> seen(N, 0);
+        for (uint64_t r = 0; r < N; ++r) {
+            if (seen[r]) continue;
+            seen[r] = 1;
+            size_t head = bfs.size();
+            bfs.push_back((uint32_t)r);
+            while (head < bfs.size()) {
+                const uint32_t u = bfs[head++];
+                for (uint64_t a = g.row_ptr[u]; a < g.row_ptr[u + 1]; ++a) {
+                    const uint32_t v = g.adj[a];
+                    if (!seen[v]) { seen[v] = 1; bfs.push_back(v); }
+                }
+            }
         }
     }
-    // sliced ELL: slice s of the whole position space = positions 32 s .. 32 s + 31, row length deg[32 s]
+    // Positions: class-major; inside a class the sites keep the BFS order, except that every window of
+    // SG_SORT_WINDOW consecutive sites is stably sorted by degree, so that the 32 sites of a slice have (almost
+    // always) one degree and the sliced-ELL rows carry ~1 % padding.  Classes start at multiples of 32; the gap
+    // positions are padding (orig = NONE, spin word 0, never written).
+    std::vector<uint64_t> ccount(K, 0);
+    for (uint64_t i = 0; i < N; ++i) ccount[g.colour[i]]++;
+    g.cls.assign(K, VBClass{});
+    uint64_t P = 0;
+    for (uint32_t k = 0; k < K; ++k) {
+        g.cls[k].pos0 = P;
+        g.cls[k].n = (ccount[k] + 31) / 32 * 32;
+        P += g.cls[k].n;
+    }
+    if (P >= (1ull << 31)) { sg_set_error("sg_create: too many sites"); return false; }
+    g.P = P;
+    g.orig.assign(P, SG_NONE); g.pos.resize(N); g.deg.assign(P, 0);
+    {
+        std::vector<uint64_t> fill(K);
+        for (uint32_t k = 0; k < K; ++k) fill[k] = g.cls[k].pos0;
+        for (uint64_t q = 0; q < N; ++q) g.orig[fill[g.colour[bfs[q]]]++] = bfs[q];
+        std::vector<uint32_t> tmp(SG_SORT_WINDOW);
+        for (uint32_t k = 0; k < K; ++k) {
+            const uint64_t p0 = g.cls[k].pos0, p1 = p0 + ccount[k];
+            for (uint64_t w0 = p0; w0 < p1; w0 += SG_SORT_WINDOW) {
+                const uint64_t w1 = std::min<uint64_t>(p1, w0 + SG_SORT_WINDOW);
+                uint32_t hist[33] = {0};
+                for (uint64_t p = w0; p < w1; ++p) hist[g.row_ptr[g.orig[p] + 1] - g.row_ptr[g.orig[p]] + 1]++;
+                for (int d = 0; d < 32; ++d) hist[d + 1] += hist[d];
+                for (uint64_t p = w0; p < w1; ++p) tmp[hist[g.row_ptr[g.orig[p] + 1] - g.row_ptr[g.orig[p]]]++] = g.orig[p];
+                std::copy(tmp.begin(), tmp.begin() + (w1 - w0), g.orig.begin() + w0);
+            }
+        }
+        for (uint64_t p = 0; p < P; ++p)
+            if (g.orig[p] != SG_NONE) {
+                g.pos[g.orig[p]] = (uint32_t)p;
+                g.deg[p] = (uint8_t)(g.row_ptr[g.orig[p] + 1] - g.row_ptr[g.orig[p]]);
+            }
+    }
+    std::vector<uint32_t>().swap(bfs);
+    // sliced ELL: slice s = positions 32 s .. 32 s + 31, row length = the largest degree in the slice
     const uint64_t nslices = P / 32;
     g.slice_ptr.assign(nslices + 1, 0);
     for (uint64_t s = 0; s < nslices; ++s) {
-        const uint64_t next = (uint64_t)g.slice_ptr[s] + g.deg[32 * s];
+        uint32_t D = 0;
+        for (uint32_t j = 0; j < 32; ++j) D = std::max<uint32_t>(D, g.deg[32 * s + j]);
+        const uint64_t next = (uint64_t)g.slice_ptr[s] + D;
         if (next > 0x7FFFFFFull) { sg_set_error("sg_create: instance too large for 32-bit entry indices"); return false; }
         g.slice_ptr[s + 1] = (uint32_t)next;
     }
@@ -177,41 +219,20 @@ bool sg_build_vb_graph(uint64_t N, double c, uint64_t seed, VBHostGraph &g)
         for (uint32_t j = 0; j < 32; ++j) {
             const uint64_t p = 32 * s + j;
             const uint32_t i = g.orig[p];
+            const uint32_t d = g.deg[p];
             for (uint32_t q = 0; q < D; ++q) {
                 const uint64_t ent = base + 32ull * q + j;
-                if (i != SG_NONE) {
+                if (i != SG_NONE && q < d) {
                     const uint64_t r0 = g.row_ptr[i];
                     g.col[ent] = g.pos[g.adj[r0 + q]];
                     const uint32_t e = g.adj_e[r0 + q];
                     g.eid[ent] = e;
                     if (g.eu[e] == i) g.entry_of_edge[e] = (uint32_t)ent;
                 } else {
-                    g.col[ent] = (uint32_t)p;   // padding position: points at itself, coupling word 0
+                    g.col[ent] = (uint32_t)p;   // padding entry: points at its own position, coupling word 0
                 }
             }
         }
-    }
-    // tiles for the staged sweep kernel: consecutive slices of one class, at most SG_TILE_SLICES slices
-    // and SG_TILE_ENT32 neighbour columns (32 entries each)
-    g.tiles.clear();
-    for (uint32_t k = 0; k < K; ++k) {
-        g.cls[k].tile0 = g.tiles.size();
-        uint64_t s = g.cls[k].slice0;
-        const uint64_t send = s + g.cls[k].nslices;
-        while (s < send) {
-            VBTile t{g.slice_ptr[s], (uint32_t)(32 * s), 0};
-            uint32_t ns = 0, cols = 0;
-            while (s + ns < send && ns < SG_TILE_SLICES) {
-                const uint32_t D = g.slice_ptr[s + ns + 1] - g.slice_ptr[s + ns];
-                if (ns > 0 && cols + D > SG_TILE_ENT32) break;
-                t.packed |= (uint64_t)D << (4 + 5 * ns);
-                cols += D; ++ns;
-            }
-            t.packed |= ns;
-            g.tiles.push_back(t);
-            s += ns;
-        }
-        g.cls[k].ntiles = g.tiles.size() - g.cls[k].tile0;
     }
     return true;
 }
@@ -239,13 +260,13 @@ extern "C" int sg_host_graph_info(const sg_host_graph *h, uint64_t *info)
 {
     if (!h || !info) return SG_EINVAL;
     info[0] = h->g.M; info[1] = h->g.K; info[2] = h->g.dmax; info[3] = h->g.col.size();
-    info[4] = h->g.slice_ptr.size() - 1; info[5] = h->g.N; info[6] = h->g.P; info[7] = h->g.tiles.size();
+    info[4] = h->g.slice_ptr.size() - 1; info[5] = h->g.N; info[6] = h->g.P; info[7] = SG_SORT_WINDOW;
     return SG_OK;
 }
 
 extern "C" int sg_host_graph_get(const sg_host_graph *h, uint32_t *u, uint32_t *v, uint32_t *colour, uint32_t *orig,
                                  uint32_t *deg, uint32_t *slice_ptr, uint32_t *col, uint32_t *eid,
-                                 uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0, uint64_t *tiles)
+                                 uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0)
 {
     if (!h) return SG_EINVAL;
     const VBHostGraph &g = h->g;
@@ -262,7 +283,5 @@ extern "C" int sg_host_graph_get(const sg_host_graph *h, uint32_t *u, uint32_t *
         if (class_n) class_n[k] = g.cls[k].n;
         if (class_slice0) class_slice0[k] = g.cls[k].slice0;
     }
-    if (tiles) std::memcpy(tiles, g.tiles.data(), g.tiles.size() * sizeof(VBTile));
-    if (tiles) std::memcpy(tiles, g.tiles.data(), g.tiles.size() * sizeof(VBTile));
     return SG_OK;
 }

@@ -22,30 +22,22 @@ struct Philox4 { uint32_t x[4]; };
 Philox4 sg_philox_host(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1);
 
 // ---- VB instance layout -----------------------------------------------------------------------
-// Sites are relabelled to "positions" p: sorted by (colour, degree, original label), every
-// (colour, degree) bucket starting at a multiple of 32 (gap positions are padding: orig = SG_NONE,
-// spin word 0, never written).  Slice g = positions 32g..32g+31 holds sites of one degree D and stores
-// its rows column-major (sliced ELL): the k-th neighbour of the j-th site of the slice lives at index
-// 32*slice_ptr[g] + 32*k + j of `col` (neighbour position) and, times n_words plus w, of the coupling
-// array.  Padding positions point at themselves with coupling word 0 (a satisfied bond).
+// Sites are relabelled to "positions" p: class-major (colour 0, 1, ...), every class starting at a multiple of
+// 32 (gap positions are padding: orig = SG_NONE, spin word 0, never written).  Inside a class the sites keep
+// their breadth-first index order (the locality-improving relabelling), except that every window of
+// SG_SORT_WINDOW consecutive sites is stably sorted by degree.  Slice g = positions 32g..32g+31 stores its rows
+// column-major (sliced ELL) with row length D_g = the largest degree in the slice: the k-th neighbour of the
+// j-th site of the slice lives at index 32*slice_ptr[g] + 32*k + j of `col` (neighbour position) and, times
+// n_words plus w, of the coupling array.  Entries beyond a site's degree (and all entries of padding positions)
+// point at the site's own position with coupling word 0.
 constexpr uint32_t SG_NONE = 0xFFFFFFFFu;
-constexpr uint32_t SG_TILE_SLICES = 8;    // slices (of 32 positions) per tile of the staged sweep kernel
-constexpr uint32_t SG_TILE_ENT32 = 32;    // neighbour columns (32 entries each) per tile: 1024 entries
+constexpr uint32_t SG_SORT_WINDOW = 4096;
 
 struct VBClass {
     uint64_t pos0;     // first position of the class (multiple of 32)
     uint64_t n;        // positions in the class, padding included (multiple of 32)
     uint64_t slice0;   // first slice = pos0 / 32
     uint64_t nslices;  // n / 32
-    uint64_t tile0;    // first tile
-    uint64_t ntiles;
-};
-
-// A tile = up to 8 consecutive slices of one class.  16 bytes, read by the staged sweep kernel.
-struct VBTile {
-    uint32_t ent32;    // first neighbour column (entry index / 32)
-    uint32_t pos0;     // first position
-    uint64_t packed;   // bits 0-3: number of slices; bits 4+5s .. 8+5s: row length of slice s
 };
 
 struct VBHostGraph {
@@ -63,8 +55,7 @@ struct VBHostGraph {
     std::vector<uint32_t> slice_ptr;       // nslices_total+1, units of 32 entries
     std::vector<uint32_t> col;             // 32*slice_ptr.back() entries: neighbour positions
     std::vector<uint32_t> eid;             // same length: edge id or 0xFFFFFFFF for padding
-    std::vector<uint8_t> deg;              // per position (padding positions: the degree of their bucket)
-    std::vector<VBTile> tiles;
+    std::vector<uint8_t> deg;              // per position (padding positions: 0)
     std::vector<uint32_t> entry_of_edge;   // M: entry index of edge e at endpoint eu[e]
 };
 
@@ -80,21 +71,17 @@ struct VBDevice {
     uint64_t *J = nullptr;          // entries*W coupling words
     uint32_t *col = nullptr;        // entries
     uint32_t *orig = nullptr;       // P (SG_NONE = padding)
-    VBTile *tiles = nullptr;
     uint32_t *slice_ptr = nullptr;  // nslices+1
     uint64_t *thr = nullptr;        // 32 thresholds (thr[k], k=0..31; beyond dmax = 0)
-    uint32_t dhot = 0;              // sites with degree >= dhot are kept in L2 (evict_last); bit 31 of col marks such neighbours
 };
 
 struct SGSeed { uint32_t k0, k1; };
 
 int sgk_init_spins(uint64_t *spin, const uint32_t *orig, uint64_t N, uint32_t W, SGSeed key, cudaStream_t st);
 int sgk_init_vb_couplings(uint64_t *J, const uint32_t *eid, uint64_t entries, uint32_t W, SGSeed key, cudaStream_t st);
-bool sgk_vb_sweep_staged_ok(uint64_t P, uint64_t entries, uint32_t W);
-int sgk_vb_sweep_class_staged(const VBDevice &d, const VBClass &c, uint64_t sweep, SGSeed key, cudaStream_t st);
-bool sgk_vb_sweep_fast_ok(uint64_t N, uint64_t entries, uint32_t W);
-int sgk_vb_sweep_class_fast(const VBDevice &d, const VBClass &c, uint32_t W, uint64_t sweep, SGSeed key, cudaStream_t st);
-int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint32_t W, uint64_t sweep, SGSeed key, cudaStream_t st);
+// one colour class of one sweep; P, entries = sizes of the whole instance (choose 32- or 64-bit index arithmetic)
+int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint64_t P, uint64_t entries, uint32_t W, uint64_t sweep, SGSeed key,
+                       cudaStream_t st);
 // counts[64*W] (device, u64) += per-lane number of set bits of (a XOR b) over n_sites*W words
 int sgk_xor_popcount(const uint64_t *a, const uint64_t *b, uint64_t n_sites, uint32_t W, uint64_t *counts, cudaStream_t st);
 // counts[64*W] += per-lane sum over the class's sites of u_i (unsatisfied incident bonds)

@@ -1,6 +1,6 @@
-// sg_kernels.cu -- CUDA kernels (sm_100a) of the Viana-Bray path: initial spins and couplings,
-// the colour-class Metropolis sweep (row a3 of SURVEY.md 8(a)), the
-// correlation counts (a6) and the energy (a7).
+// sg_kernels.cu -- CUDA kernels (sm_100a) of the Viana-Bray path besides the sweep (sg_vb_sweep.cu):
+// initial spins and couplings (a1, a2 of SURVEY.md 8(a)), the correlation counts (a6)
+// and the energy (a7).
 // Conventions: DESIGN.md section 3.  All arithmetic is integer / bitwise.
 #include <cuda_runtime.h>
 
@@ -146,58 +146,6 @@ __device__ __forceinline__ uint64_t lanes_ge(const Planes5 &P, uint32_t umin)
         eq &= ~(pl[b] ^ cb);
     }
     return gt | eq;
-}
-
-__global__ void __launch_bounds__(256)
-k_vb_sweep(uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, const uint32_t *__restrict__ col,
-           const uint32_t *__restrict__ orig, const uint32_t *__restrict__ slice_ptr,
-           const uint64_t *__restrict__ thr, uint64_t pos0, uint64_t n_sites, uint64_t slice0, uint64_t nslices,
-           uint32_t W, uint32_t sweep_lo, uint32_t sweep_hi, uint32_t k0, uint32_t k1)
-{
-    const uint64_t T = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const uint32_t per_slice = 32u * W;
-    const uint64_t slice = T / per_slice;
-    if (slice >= nslices) return;
-    const uint32_t t = (uint32_t)(T % per_slice);
-    const uint32_t j = t / W, w = t % W;
-    const uint64_t local = slice * 32 + j;
-    if (local >= n_sites) return;
-    const uint64_t p = pos0 + local;
-    const uint64_t pol_stream = policy_evict_first();
-    const uint64_t pol_keep = policy_evict_last();
-
-    const uint32_t sp0 = __ldg(slice_ptr + slice0 + slice), sp1 = __ldg(slice_ptr + slice0 + slice + 1);
-    const uint32_t D = sp1 - sp0;
-    uint64_t *own_ptr = spin + p * W + w;
-    const uint64_t own = ld_keep_u64(own_ptr, pol_keep);
-    const uint32_t d = D;   // slices hold sites of one degree
-    const uint32_t site = ld_stream_u32(orig + p, pol_stream);
-    if (site == SG_NONE) return;   // padding position
-
-    const Planes5 P = count_unsatisfied<true>(spin, J, col, 32ull * sp0, D, j, t, w, W, own, pol_stream, pol_keep);
-
-    // Metropolis uniform shared by the 64 lanes: r = x_{w&3} of P(site, w>>2, sweep, tag 0)
-    uint32_t x[4];
-    philox4x32_10(site, w >> 2, sweep_lo, sweep_hi /* tag 0 */, k0, k1, x);
-    const uint32_t r = (w & 2u) ? ((w & 1u) ? x[3] : x[2]) : ((w & 1u) ? x[1] : x[0]);
-    // thr[k] is non-increasing in k, so r < thr[kk]  <=>  kk <= kstar := #{k>=1 : r < thr[k]}.
-    // flip  <=>  kk = d - 2u <= kstar  <=>  u >= ceil((d - kstar)/2)
-    uint32_t kstar = 0;
-    while (kstar < d && (uint64_t)r < __ldg(thr + kstar + 1)) ++kstar;
-    const uint32_t umin = (d - kstar + 1u) >> 1;
-    const uint64_t flip = lanes_ge(P, umin);
-    st_keep_u64(own_ptr, own ^ flip, pol_keep);
-}
-
-int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint32_t W, uint64_t sweep, SGSeed key, cudaStream_t st)
-{
-    if (c.n == 0) return SG_OK;
-    const uint64_t threads = c.nslices * 32ull * W;
-    const unsigned grid = (unsigned)((threads + 255) / 256);
-    k_vb_sweep<<<grid, 256, 0, st>>>(d.spin, d.J, d.col, d.orig, d.slice_ptr, d.thr, c.pos0, c.n, c.slice0,
-                                     c.nslices, W, (uint32_t)sweep, (uint32_t)(sweep >> 32) /* tag 0 */, key.k0, key.k1);
-    SG_LAUNCH_CHECK();
-    return SG_OK;
 }
 
 // ------------------------------------------------------------------------------------ per-lane counting

@@ -19,8 +19,7 @@ struct sg_sim {
     VBHostGraph g;
     VBDevice vb;
     std::vector<uint64_t> thr_host;
-    bool vb_staged = false;                  // persistent TMA-staged sweep kernel usable (n_words = 1)
-    bool vb_fast = false;                    // specialised sweep kernel usable for this shape
+    uint64_t vb_entries = 0;                 // sliced-ELL entries (padding included)
     // SK
     SKDevice sk;
     // common
