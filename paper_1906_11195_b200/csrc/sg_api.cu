@@ -110,7 +110,8 @@ extern "C" int sg_sweep(sg_sim *h, uint64_t n)
     cudaStream_t st = sgx_stream();
     for (uint64_t it = 0; it < n; ++it) {
         for (uint32_t k = 0; k < h->g.K; ++k) {
-            const int rc = sgk_vb_sweep_class(h->vb, h->g.cls[k], h->g.P, h->vb_entries, h->W, h->sweep, h->key, st);
+            const int rc = sgk_vb_sweep_class(h->vb, h->g.cls[k], h->g.P, h->vb_entries, h->W, h->sweep, h->key, h->vb_reverse, st);
+            h->vb_reverse = !h->vb_reverse;
             if (rc) return rc;
         }
         h->sweep++;

@@ -78,3 +78,9 @@ __device__ __forceinline__ uint64_t ld_plain_u64(const uint64_t *ptr)
     asm volatile("ld.global.b64 %0, [%1];" : "=l"(v) : "l"(ptr));
     return v;
 }
+
+// pull [ptr, ptr + bytes) from HBM into L2 (bytes a multiple of 16, ptr 16-byte aligned); no data is returned
+__device__ __forceinline__ void bulk_prefetch_l2(const void *ptr, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(ptr), "r"(bytes) : "memory");
+}

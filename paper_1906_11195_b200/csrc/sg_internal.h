@@ -79,9 +79,10 @@ struct SGSeed { uint32_t k0, k1; };
 
 int sgk_init_spins(uint64_t *spin, const uint32_t *orig, uint64_t N, uint32_t W, SGSeed key, cudaStream_t st);
 int sgk_init_vb_couplings(uint64_t *J, const uint32_t *eid, uint64_t entries, uint32_t W, SGSeed key, cudaStream_t st);
-// one colour class of one sweep; P, entries = sizes of the whole instance (choose 32- or 64-bit index arithmetic)
+// one colour class of one sweep; P, entries = sizes of the whole instance (choose 32- or 64-bit index arithmetic);
+// reverse = walk the class from its last slice to its first (callers alternate it from launch to launch)
 int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint64_t P, uint64_t entries, uint32_t W, uint64_t sweep, SGSeed key,
-                       cudaStream_t st);
+                       bool reverse, cudaStream_t st);
 // counts[64*W] (device, u64) += per-lane number of set bits of (a XOR b) over n_sites*W words
 int sgk_xor_popcount(const uint64_t *a, const uint64_t *b, uint64_t n_sites, uint32_t W, uint64_t *counts, cudaStream_t st);
 // counts[64*W] += per-lane sum over the class's sites of u_i (unsatisfied incident bonds)

@@ -34,11 +34,14 @@ template <int LOGW, bool WIDE, int MINB>
 __global__ void __launch_bounds__(256, MINB)
 k_vb_sweep(uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, const uint32_t *__restrict__ col,
            const uint32_t *__restrict__ orig, const uint32_t *__restrict__ slice_ptr, const uint64_t *__restrict__ thr,
-           uint32_t pos0, uint32_t slice0, uint32_t nslices, uint32_t Wrt, uint32_t sweep_lo, uint32_t sweep_hi, uint32_t k0, uint32_t k1)
+           uint32_t pos0, uint32_t slice0, uint32_t nslices, uint32_t Wrt, uint32_t sweep_lo, uint32_t sweep_hi, uint32_t k0, uint32_t k1,
+           uint32_t reverse)
 {
     using I = typename Idx<WIDE>::type;
     const uint32_t W = LOGW >= 0 ? (1u << (LOGW >= 0 ? LOGW : 0)) : Wrt;
-    const I T = (I)blockIdx.x * 256u + threadIdx.x;
+    // `reverse`: walk the class from its last slice to its first (the host alternates the direction from launch to
+    // launch, so that a launch starts where the previous one ended and finds those spin words still in L2)
+    const I T = (I)(reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x) * 256u + threadIdx.x;
     const uint32_t per_slice = 32u * W;
     const uint32_t slice = LOGW >= 0 ? (uint32_t)(T >> (5 + (LOGW >= 0 ? LOGW : 0))) : (uint32_t)(T / per_slice);
     if (slice >= nslices) return;
@@ -116,12 +119,13 @@ k_vb_sweep(uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, const ui
 }
 
 template <int LOGW, bool WIDE, int MINB>
-int launch(const VBDevice &d, const VBClass &c, uint32_t W, uint64_t sweep, SGSeed key, cudaStream_t st)
+int launch(const VBDevice &d, const VBClass &c, uint32_t W, uint64_t sweep, SGSeed key, bool reverse, cudaStream_t st)
 {
     const uint64_t threads = c.nslices * 32ull * W;
     const unsigned grid = (unsigned)((threads + 255) / 256);
     k_vb_sweep<LOGW, WIDE, MINB><<<grid, 256, 0, st>>>(d.spin, d.J, d.col, d.orig, d.slice_ptr, d.thr, (uint32_t)c.pos0, (uint32_t)c.slice0,
-                                                       (uint32_t)c.nslices, W, (uint32_t)sweep, (uint32_t)(sweep >> 32) /* tag 0 */, key.k0, key.k1);
+                                                       (uint32_t)c.nslices, W, (uint32_t)sweep, (uint32_t)(sweep >> 32) /* tag 0 */, key.k0, key.k1,
+                                                       reverse ? 1u : 0u);
     sgk_count_launch();
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) {
@@ -134,20 +138,21 @@ int launch(const VBDevice &d, const VBClass &c, uint32_t W, uint64_t sweep, SGSe
 }  // namespace
 
 int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint64_t P, uint64_t entries, uint32_t W, uint64_t sweep, SGSeed key,
-                       cudaStream_t st)
+                       bool reverse, cudaStream_t st)
 {
     if (c.n == 0) return SG_OK;
     if (c.nslices * 32ull * W >= (1ull << 40)) { sg_set_error("sgk_vb_sweep_class: class too large"); return SG_EINVAL; }
     const bool narrow = P * W < (1ull << 32) && entries * W < (1ull << 32);
+    // 5 CTAs of 256 threads per SM: 48 registers, no spills (6 CTAs spill, 4 lose latency hiding; profiles/r01_sweep.md)
     if (narrow) {
         switch (W) {
-        case 1: return launch<0, false, 6>(d, c, W, sweep, key, st);
-        case 2: return launch<1, false, 6>(d, c, W, sweep, key, st);
-        case 4: return launch<2, false, 6>(d, c, W, sweep, key, st);
-        case 8: return launch<3, false, 6>(d, c, W, sweep, key, st);
-        case 16: return launch<4, false, 6>(d, c, W, sweep, key, st);
-        default: return launch<-1, false, 4>(d, c, W, sweep, key, st);
+        case 1: return launch<0, false, 5>(d, c, W, sweep, key, reverse, st);
+        case 2: return launch<1, false, 5>(d, c, W, sweep, key, reverse, st);
+        case 4: return launch<2, false, 5>(d, c, W, sweep, key, reverse, st);
+        case 8: return launch<3, false, 5>(d, c, W, sweep, key, reverse, st);
+        case 16: return launch<4, false, 5>(d, c, W, sweep, key, reverse, st);
+        default: return launch<-1, false, 4>(d, c, W, sweep, key, reverse, st);
         }
     }
-    return launch<-1, true, 4>(d, c, W, sweep, key, st);
+    return launch<-1, true, 4>(d, c, W, sweep, key, reverse, st);
 }
