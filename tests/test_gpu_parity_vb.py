@@ -181,15 +181,54 @@ def test_word_independence(sg):
     assert np.array_equal(a.energy(), b.energy()[:256])
 
 
-@pytest.mark.parametrize("kernel", ["staged", "fast", "general"])
+@pytest.mark.parametrize("order", ["label", "bfs"])
 @pytest.mark.parametrize("N,c,T,seed", [(1 << 14, 4.0, 1.0, 3), (5000, 9.0, 1.4, 4), (100, 4.0, 0.6, 5)])
-def test_every_sweep_kernel_variant_matches_oracle(sg, oracle_mod, monkeypatch, kernel, N, c, T, seed):
-    """n_words = 1 has three implementations of the sweep (persistent TMA-staged, thread-per-site,
-    general-W); SG_VB_KERNEL picks one at sg_create.  All must equal the oracle."""
-    monkeypatch.setenv("SG_VB_KERNEL", kernel)
+def test_relabelling_does_not_change_any_output(sg, oracle_mod, monkeypatch, order, N, c, T, seed):
+    """P11 / Q15: the internal relabelling (breadth-first order, or plain label order with SG_VB_ORDER=label)
+    changes no output, because the Philox counter uses the original label."""
+    monkeypatch.setenv("SG_VB_ORDER", order)
     g, o = _pair(sg, oracle_mod, N, c, T, seed, 1)
+    g.snapshot(1); o.snapshot(1)
     for _ in range(4):
         g.sweep(2)
         o.sweep(2)
         _assert_same_state(g, o)
     assert np.array_equal(g.energy(), o.energy())
+    assert np.array_equal(g.correlation(1), o.correlation(1))
+
+
+def _lane_counts(x):
+    """per-lane popcount over sites of an (N, W) uint64 array -> 64*W counts (plain numpy, no oracle, no CUDA)"""
+    out = np.zeros(64 * x.shape[1], dtype=np.uint64)
+    for w in range(x.shape[1]):
+        col = np.ascontiguousarray(x[:, w])
+        for b in range(64):
+            out[64 * w + b] = int(((col >> np.uint64(b)) & np.uint64(1)).sum())
+    return out
+
+
+def test_full_size_config3_late_sweep(sg, oracle_mod):
+    """BASELINE.json configs[2] at full size (N = 2^24, W = 1, T = 1), in the launch configuration bench.py times:
+    the GPU runs 40 sweeps, then ONE more sweep is compared element by element with the oracle started from the
+    GPU's state at sweep 40 (a sweep is a pure function of (state, index), Q15), together with the
+    correlation counts against a snapshot and the energy change (oracle's accumulated dE of that sweep)."""
+    N, W, T0 = 1 << 24, 1, 40
+    g = sg.Sim(sg.SG_MODEL_VB, N, 4.0, 1.0, 1, W)
+    o = oracle_mod.Oracle(oracle_mod.VB, N, 4.0, 1.0, 1, W)
+    assert g.M == o.M and g.n_colours == o.n_colours and g.max_degree == o.max_degree
+    assert np.array_equal(g.spins(), o.spins())                   # initial configuration
+    idx = np.random.default_rng(1).integers(0, g.M, size=200000)
+    assert np.array_equal(g.couplings()[idx], o.couplings()[idx])
+    g.sweep(T0)
+    before = g.spins()
+    E_before = g.energy()
+    g.snapshot(0)
+    o.set_spins(before)
+    o.set_sweep_count(T0)
+    dE0 = o.accumulated_dE().copy()
+    g.sweep(1)
+    o.sweep(1)
+    after = g.spins()
+    assert np.array_equal(after, o.spins())
+    assert np.array_equal(g.energy() - E_before, o.accumulated_dE() - dE0)
+    assert np.array_equal(g.correlation(0), _lane_counts(before ^ after))
