@@ -79,8 +79,7 @@ __device__ __forceinline__ uint64_t ld_plain_u64(const uint64_t *ptr)
     return v;
 }
 
-// pull [ptr, ptr + bytes) from HBM into L2 (bytes a multiple of 16, ptr 16-byte aligned); no data is returned
-__device__ __forceinline__ void bulk_prefetch_l2(const void *ptr, uint32_t bytes)
-{
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(ptr), "r"(bytes) : "memory");
-}
+// Programmatic dependent launch (sm_90+): wait until the grid this one depends on has completed and its memory
+// operations are visible; allow the grid that depends on this one to start launching.
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }

@@ -38,33 +38,31 @@ k_vb_sweep(uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, const ui
            uint32_t reverse)
 {
     using I = typename Idx<WIDE>::type;
+    const uint32_t bid = reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
     const uint32_t W = LOGW >= 0 ? (1u << (LOGW >= 0 ? LOGW : 0)) : Wrt;
     // `reverse`: walk the class from its last slice to its first (the host alternates the direction from launch to
     // launch, so that a launch starts where the previous one ended and finds those spin words still in L2)
-    const I T = (I)(reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x) * 256u + threadIdx.x;
+    const I T = (I)bid * 256u + threadIdx.x;
     const uint32_t per_slice = 32u * W;
     const uint32_t slice = LOGW >= 0 ? (uint32_t)(T >> (5 + (LOGW >= 0 ? LOGW : 0))) : (uint32_t)(T / per_slice);
-    if (slice >= nslices) return;
+    // (no thread leaves before griddep_wait(): ptxas hoists the wait above every load that follows an exit)
+    const bool in_range = slice < nslices;
     const uint32_t t = LOGW >= 0 ? (uint32_t)T & (per_slice - 1u) : (uint32_t)(T % per_slice);
     const uint32_t j = LOGW >= 0 ? t >> (LOGW >= 0 ? LOGW : 0) : t / W;
     const uint32_t w = LOGW >= 0 ? t & (W - 1u) : t % W;
     const uint32_t p = pos0 + slice * 32u + j;
     const uint64_t pol_stream = policy_evict_first();
 
-    const uint32_t site = ld_stream_u32(orig + p, pol_stream);
-    if (site == SG_NONE) return;   // padding position
-    const uint32_t sp0 = __ldg(slice_ptr + slice0 + slice), sp1 = __ldg(slice_ptr + slice0 + slice + 1);
-    const uint32_t D = sp1 - sp0;  // row length of the slice >= degree of this site
+    const uint32_t site = in_range ? ld_stream_u32(orig + p, pol_stream) : SG_NONE;   // SG_NONE: padding position
+    uint32_t sp0 = 0, sp1 = 0;
+    if (in_range) { sp0 = __ldg(slice_ptr + slice0 + slice); sp1 = __ldg(slice_ptr + slice0 + slice + 1); }
+    const uint32_t D = site != SG_NONE ? sp1 - sp0 : 0u;  // row length of the slice >= degree of this site
     uint64_t *own_ptr = spin + (I)p * W + w;
-    const uint64_t own = *own_ptr;
 
     const uint32_t *cp = col + (I)sp0 * 32u + j;          // + 32 per neighbour slot
     const uint64_t *jp = J + (I)sp0 * 32u * W + t;         // + 32 W per neighbour slot
-    uint64_t p0 = 0, p1 = 0, p2 = 0, p3 = 0, p4 = 0;
-    uint32_t d = 0;
-    for (uint32_t k = 0; k < D; k += 4) {
-        uint32_t nb[4];
-        uint64_t jw[4], sn[4];
+    // neighbour indices and coupling words of slots k .. k+3 (padding: own position, coupling 0)
+    auto load_chunk = [&](uint32_t k, uint32_t (&nb)[4], uint64_t (&jw)[4]) {
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             nb[q] = p;
@@ -74,14 +72,34 @@ k_vb_sweep(uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, const ui
                 jw[q] = ld_stream_u64(jp + (I)(k + q) * per_slice, pol_stream);
             }
         }
+    };
+    uint32_t nb[4];
+    uint64_t jw[4];
+    load_chunk(0, nb, jw);
+    // Everything above reads arrays that no kernel writes.  The launch is a programmatic dependent launch: this
+    // grid's CTAs start while the previous colour class is still draining and wait here, before the first spin
+    // word is read, until that grid has completed and its writes are visible.
+    // (ptxas hoists the wait above every global load that no thread exit separates from it; this exit, never taken
+    // because indices are positions < 2^31, depends on the row loads and so pins them before the wait)
+    if ((nb[0] & nb[1] & nb[2] & nb[3]) == SG_NONE || site == SG_NONE) return;
+    griddep_wait();
+    griddep_launch_dependents();
+    const uint64_t own = *own_ptr;
+
+    uint64_t p0 = 0, p1 = 0, p2 = 0, p3 = 0, p4 = 0;
+    uint32_t d = 0;
+    for (uint32_t k = 0; k < D; k += 4) {
+        uint64_t sn[4], jc[4];
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             sn[q] = own;                                   // padding entry: own ^ own ^ 0 = satisfied
+            jc[q] = jw[q];
             if (nb[q] != p) { sn[q] = spin[(I)nb[q] * W + w]; ++d; }
         }
+        if (k + 4 < D) load_chunk(k + 4, nb, jw);          // next slots' streams go out under the gathers' latency
         uint64_t m[4];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) m[q] = own ^ sn[q] ^ jw[q];
+        for (int q = 0; q < 4; ++q) m[q] = own ^ sn[q] ^ jc[q];
         // 4 one-bit numbers -> 3 planes
         const uint64_t s = m[0] ^ m[1] ^ m[2], cy = maj64(m[0], m[1], m[2]);
         const uint64_t s0 = s ^ m[3], c2 = s & m[3];
@@ -123,11 +141,23 @@ int launch(const VBDevice &d, const VBClass &c, uint32_t W, uint64_t sweep, SGSe
 {
     const uint64_t threads = c.nslices * 32ull * W;
     const unsigned grid = (unsigned)((threads + 255) / 256);
-    k_vb_sweep<LOGW, WIDE, MINB><<<grid, 256, 0, st>>>(d.spin, d.J, d.col, d.orig, d.slice_ptr, d.thr, (uint32_t)c.pos0, (uint32_t)c.slice0,
-                                                       (uint32_t)c.nslices, W, (uint32_t)sweep, (uint32_t)(sweep >> 32) /* tag 0 */, key.k0, key.k1,
-                                                       reverse ? 1u : 0u);
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(256);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see griddep_wait() in the kernel
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    static const bool no_pdl = std::getenv("SG_NO_PDL") != nullptr;   // measurement knob
+    cfg.numAttrs = no_pdl ? 0 : 1;
+    const cudaError_t le = cudaLaunchKernelEx(&cfg, k_vb_sweep<LOGW, WIDE, MINB>, d.spin, (const uint64_t *)d.J, (const uint32_t *)d.col,
+                                              (const uint32_t *)d.orig, (const uint32_t *)d.slice_ptr, (const uint64_t *)d.thr, (uint32_t)c.pos0,
+                                              (uint32_t)c.slice0, (uint32_t)c.nslices, W, (uint32_t)sweep, (uint32_t)(sweep >> 32) /* tag 0 */,
+                                              key.k0, key.k1, reverse ? 1u : 0u);
     sgk_count_launch();
-    const cudaError_t e = cudaGetLastError();
+    const cudaError_t e = le != cudaSuccess ? le : cudaGetLastError();
     if (e != cudaSuccess) {
         sg_set_error(std::string("k_vb_sweep launch failed: ") + cudaGetErrorString(e));
         return SG_ECUDA;
