@@ -240,10 +240,10 @@ def run_ours(args):
         "vs_baseline": None, "dtype": "u64", "data": "synthetic",
         "config": {"workload": f"VB N=2^{args.log2n} c=4 W={W} T={args.T} seed=1+rank (BASELINE.json configs[2])",
                    "step": f"sg_sweep({SWEEPS_PER_STEP}) + sg_snapshot + sg_correlation + sg_energy",
-                   "l2": "inputs larger than L2 (couplings+indices 768 MiB, spins 128 MiB streamed every sweep)",
+                   "l2": "inputs larger than L2: every sweep streams 777 MiB of couplings+indices+labels and reads/writes the 128 MiB spin array (L2 126 MiB); no flush needed",
                    "parallelism": "replicas sharded by sample word, no data-path collective" if world > 1 else "single GPU",
                    "create_s": round(create_s, 2)},
-        "roofline": {"bound": "hbm", "kernel": "k_vb_sweep (all colour classes of a sweep)", "achieved": achieved, "peak": peak,
+        "roofline": {"bound": "hbm", "kernel": "k_vb_sweep (the 6-7 colour-class launches of a sweep)", "achieved": achieved, "peak": peak,
                      "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                      "bytes_per_site_word": BYTES_PER_SITE_WORD, "sweep_ms": sweep_ms / (SWEEPS_PER_STEP * args.steps),
                      "sweep_share_of_step": sweep_ms / ms},

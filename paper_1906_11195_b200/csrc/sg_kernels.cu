@@ -272,27 +272,36 @@ int sgk_xor_popcount(const uint64_t *a, const uint64_t *b, uint64_t n_sites, uin
 
 // ------------------------------------------------------------------------------------ VB energy
 // counts[w*64+b] += sum over the class's sites of u_i (unsatisfied incident bonds of lane w*64+b).
-// sum over all classes = 2 U_l, and E_l = 2 U_l - M.  One warp per slice-row of 32 threads,
-// striding over the class's thread range; same thread -> (slice, j, w) map as the sweep.
-__global__ void __launch_bounds__(256)
+// sum over all classes = 2 U_l, and E_l = 2 U_l - M.  One warp per slice-row of 32 threads, UNSAT_ROWS rows per
+// warp; same thread -> (slice, j, w) map as the sweep.  Per-lane totals go
+// to shared-memory counters first and to global memory once per CTA.
+constexpr uint32_t UNSAT_ROWS = 4;
+constexpr uint32_t UNSAT_SMEM_WORDS = 32;   // contiguous path: n_words <= 32
+
+__global__ void __launch_bounds__(256, 3)
 k_vb_unsat(const uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, const uint32_t *__restrict__ col,
            const uint32_t *__restrict__ slice_ptr, uint64_t pos0, uint64_t n_sites, uint64_t slice0, uint64_t nslices,
            uint32_t W, unsigned long long *__restrict__ counts)
 {
-    constexpr int P = 10, PT = P + 5;   // 32 additions of values <= 31 fit in 10 planes
+    constexpr int P = 3, PT = P + 5 + 5;   // UNSAT_ROWS additions of values <= 31, then 5 doublings in the warp
+    __shared__ unsigned long long s_counts[64 * UNSAT_SMEM_WORDS];
+    const bool contig = W <= UNSAT_SMEM_WORDS && (W & (W - 1)) == 0;
+    if (contig) {
+        for (uint32_t q = threadIdx.x; q < 64u * W; q += blockDim.x) s_counts[q] = 0;
+        __syncthreads();
+    }
     uint64_t acc[PT];
     vc_clear(acc);
     const uint32_t lane = threadIdx.x & 31u;
     const uint64_t warp = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const uint64_t nwarps = ((uint64_t)gridDim.x * blockDim.x) >> 5;
     const uint64_t pol_stream = policy_evict_first();
-    const uint64_t pol_keep = policy_evict_last();
+    const uint64_t pol_keep = policy_evict_normal();
     const uint32_t per_slice = 32u * W;
     const uint64_t nrows = nslices * W;           // warp-rows of 32 threads
-    const bool contig = W <= 32 && (W & (W - 1)) == 0;
-    uint32_t pending = 0;
-    uint32_t w_last = 0;
-    for (uint64_t row = warp; row < nrows; row += nwarps) {
+#pragma unroll 1
+    for (uint32_t it = 0; it < UNSAT_ROWS; ++it) {
+        const uint64_t row = warp * UNSAT_ROWS + it;
+        if (row >= nrows) break;
         const uint64_t T = row * 32 + lane;
         const uint64_t slice = T / per_slice;
         const uint32_t t = (uint32_t)(T % per_slice);
@@ -306,16 +315,10 @@ k_vb_unsat(const uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, co
             u = count_unsatisfied<false>(spin, J, col, 32ull * sp0, sp1 - sp0, j, t, w, W, own, pol_stream, pol_keep);
         }
         if (contig) {
-            vc_add_planes5<P, PT>(acc, u);
-            if (++pending == 32) {
-                vc_warp_flush<PT>(acc, W, 0, counts);
-                vc_clear(acc);
-                pending = 0;
-            }
+            vc_add_planes5<P + 5, PT>(acc, u);
         } else {
             // arbitrary W: lanes of a warp hold different words with no shuffle-friendly pattern;
             // flush every lane on its own (slow path, exact).
-            (void)w_last;
             const uint64_t pl[5] = {u.p0, u.p1, u.p2, u.p3, u.p4};
             for (int b = 0; b < 64; ++b) {
                 unsigned long long v = 0;
@@ -325,16 +328,19 @@ k_vb_unsat(const uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, co
             }
         }
     }
-    if (contig && pending) vc_warp_flush<PT>(acc, W, 0, counts);
+    if (contig) {
+        vc_warp_flush<PT>(acc, W, 0, s_counts);
+        __syncthreads();
+        for (uint32_t q = threadIdx.x; q < 64u * W; q += blockDim.x)
+            if (s_counts[q]) atomicAdd(counts + q, s_counts[q]);
+    }
 }
 
 int sgk_vb_unsat_class(const VBDevice &d, const VBClass &c, uint32_t W, uint64_t *counts, cudaStream_t st)
 {
     if (c.n == 0) return SG_OK;
     const uint64_t rows = c.nslices * W;
-    uint64_t blocks = (rows + 8 * 8 - 1) / (8 * 8);
-    if (blocks > 148 * 8) blocks = 148 * 8;
-    if (blocks < 1) blocks = 1;
+    const uint64_t blocks = (rows + 8 * UNSAT_ROWS - 1) / (8 * UNSAT_ROWS);
     k_vb_unsat<<<(unsigned)blocks, 256, 0, st>>>(d.spin, d.J, d.col, d.slice_ptr, c.pos0, c.n, c.slice0, c.nslices, W,
                                                  (unsigned long long *)counts);
     SG_LAUNCH_CHECK();
