@@ -157,7 +157,10 @@ def run_ours(args):
 
     N, W = 1 << args.log2n, args.n_words
     t0 = time.perf_counter()
-    sim = sg.Sim(sg.SG_MODEL_VB, N, 4.0, args.T, 1 + rank, W)
+    from paper_1906_11195_b200.workloads import Workload, shard
+
+    wl = shard(Workload("bench", sg.SG_MODEL_VB, N, 4.0, args.T, 1, W, 0), rank, world)
+    sim = sg.Sim(wl.model, wl.N, wl.c, wl.T, wl.seed, wl.n_words)
     create_s = time.perf_counter() - t0
     counts = np.zeros(64 * W, dtype=np.uint64)
     energy = np.zeros(64 * W, dtype=np.int64)

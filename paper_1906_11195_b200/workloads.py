@@ -76,3 +76,16 @@ def run_schedule(sim, total_sweeps: int):
     if now < total_sweeps:
         sim.sweep(total_sweeps - now)
     return out
+
+
+def shard(w: Workload, rank: int, world: int) -> Workload:
+    """The replica rank `rank` of `world` runs: the path shards by sample, so every rank gets its
+    own n_words*64 samples of the same recipe (seed + rank); there is no data-path collective."""
+    if not 0 <= rank < world:
+        raise ValueError("rank out of range")
+    return Workload(f"{w.name}_r{rank}of{world}", w.model, w.N, w.c, w.T, w.seed + rank, w.n_words, w.sweeps)
+
+
+def global_lane(w: Workload, rank: int, lane: int) -> int:
+    """Index of a rank's lane in the job-wide, rank-major list of samples."""
+    return rank * 64 * w.n_words + lane
