@@ -38,6 +38,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--T", type=float, default=1.0)
+    ap.add_argument("--model", default="vb", choices=["vb", "sk"], help="sk: BASELINE.json configs[3] with --log2n 12 (absolute rate only)")
     ap.add_argument("--log2n", type=int, default=24)
     ap.add_argument("--n-words", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -159,7 +160,8 @@ def run_ours(args):
     t0 = time.perf_counter()
     from paper_1906_11195_b200.workloads import Workload, shard
 
-    wl = shard(Workload("bench", sg.SG_MODEL_VB, N, 4.0, args.T, 1, W, 0), rank, world)
+    model = sg.SG_MODEL_SK if args.model == "sk" else sg.SG_MODEL_VB
+    wl = shard(Workload("bench", model, N, 4.0, args.T, 1, W, 0), rank, world)
     sim = sg.Sim(wl.model, wl.N, wl.c, wl.T, wl.seed, wl.n_words)
     create_s = time.perf_counter() - t0
     counts = np.zeros(64 * W, dtype=np.uint64)
@@ -241,7 +243,8 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": "spin updates/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "u64", "data": "synthetic",
-        "config": {"workload": f"VB N=2^{args.log2n} c=4 W={W} T={args.T} seed=1+rank (BASELINE.json configs[2])",
+        "config": {"workload": (f"VB N=2^{args.log2n} c=4 W={W} T={args.T} seed=1+rank (BASELINE.json configs[2])" if args.model == "vb"
+                                else f"SK N=2^{args.log2n} W={W} T={args.T} seed=1+rank (BASELINE.json configs[3]; dependency-latency bound, roofline fields not meaningful)"),
                    "step": f"sg_sweep({SWEEPS_PER_STEP}) + sg_snapshot + sg_correlation + sg_energy",
                    "l2": "inputs larger than L2: every sweep streams 777 MiB of couplings+indices+labels and reads/writes the 128 MiB spin array (L2 126 MiB); no flush needed",
                    "parallelism": "replicas sharded by sample word, no data-path collective" if world > 1 else "single GPU",
@@ -253,9 +256,17 @@ def run_ours(args):
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
     }
     tr = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tr):
+    headline = args.model == "vb" and args.log2n == 24 and W == 1
+    if os.path.exists(tr) and headline:      # ncu dram bytes of one sweep of exactly this workload (profiles/r01_sweep.md)
         out["roofline"]["traffic"] = json.load(open(tr)).get("dram_bytes_per_sweep")
-    if not args.no_cpu_baseline:
+        out["roofline"]["per"] = "sweep (the K colour-class launches): achieved, traffic and sweep_ms are per sweep"
+    if not headline:
+        out["config"]["l2"] = "not the headline workload: see DESIGN.md section 10"
+    if args.model == "sk":
+        out["roofline"] = {"bound": "latency", "kernel": "k_sk_sweep", "achieved": None, "peak": None, "unit": None, "frac": None, "traffic": None,
+                           "note": "sequential sweep of one instance per CTA (PAPER.md:233): dependency-latency bound, absolute rate only",
+                           "sweep_ms": sweep_ms / (SWEEPS_PER_STEP * args.steps)}
+    if not args.no_cpu_baseline and args.model == "vb":
         v, dt, n = cpu_sample(args, 2)
         out["cpu_baseline"] = {"value": v, "unit": "spin updates/s", "cores": 1, "kind": "oracle", "host_cores": os.cpu_count(),
                                "sample": f"same recipe at N=2^{n.bit_length() - 1}, 2 oracle sweeps, {dt:.1f} s"}

@@ -232,3 +232,44 @@ def test_full_size_config3_late_sweep(sg, oracle_mod):
     assert np.array_equal(after, o.spins())
     assert np.array_equal(g.energy() - E_before, o.accumulated_dE() - dE0)
     assert np.array_equal(g.correlation(0), _lane_counts(before ^ after))
+
+
+def test_config2_full_size_first_sweeps(sg, oracle_mod):
+    """BASELINE.json configs[1] at full size: N = 2^20, 4 words (256 samples) per site."""
+    N, W = 1 << 20, 4
+    g, o = _pair(sg, oracle_mod, N, 4.0, 1.0, 1, W)
+    g.snapshot(0); o.snapshot(0)
+    for _ in range(2):
+        g.sweep(1)
+        o.sweep(1)
+        _assert_same_state(g, o)
+    assert np.array_equal(g.correlation(0), o.correlation(0))
+    assert np.array_equal(g.energy(), o.energy())
+
+
+@pytest.mark.parametrize("T", [float("inf"), 0.0])
+def test_largest_size_properties(sg, T):
+    """BASELINE.json configs[4] top size N = 2^26 (W = 1), where the oracle is too slow to run in a test: properties
+    that hold at any size.  T = inf: every proposal is accepted, so D alternates N, 0 and the energy is invariant (Q21);
+    T = 0: the energy never increases; always E = M (mod 2); sg_sweep(a); sg_sweep(b) = sg_sweep(a + b)."""
+    N = 1 << 26
+    g = sg.Sim(sg.SG_MODEL_VB, N, 4.0, T, 3, 1)
+    assert g.M == 2 * N
+    E0 = g.energy()
+    assert np.all((E0 - g.M) % 2 == 0)
+    g.snapshot(0)
+    g.sweep(1)
+    E1 = g.energy()
+    D1 = g.correlation(0)
+    g.sweep(2)
+    E3 = g.energy()
+    D3 = g.correlation(0)
+    assert np.all((E3 - g.M) % 2 == 0)
+    if math.isinf(T):
+        assert np.array_equal(E1, E0) and np.array_equal(E3, E0)
+        assert np.all(D1 == N) and np.all(D3 == N)
+    else:
+        assert np.all(E1 <= E0) and np.all(E3 <= E1)
+        assert np.all(D1 <= N) and np.all(D1 > 0)
+        # per-lane energy of a random +-J configuration is ~0 +- sqrt(M); a T=0 quench lowers it by O(N)
+        assert np.all(E3 < -0.5 * N)
