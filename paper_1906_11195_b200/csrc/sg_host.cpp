@@ -180,11 +180,12 @@ bool sg_build_vb_graph(uint64_t N, double c, uint64_t seed, VBHostGraph &g)
         std::vector<uint64_t> fill(K);
         for (uint32_t k = 0; k < K; ++k) fill[k] = g.cls[k].pos0;
         for (uint64_t q = 0; q < N; ++q) g.orig[fill[g.colour[bfs[q]]]++] = bfs[q];
-        std::vector<uint32_t> tmp(SG_SORT_WINDOW);
+        const uint64_t SW = SG_SORT_WINDOW;
+        std::vector<uint32_t> tmp(SW);
         for (uint32_t k = 0; k < K; ++k) {
             const uint64_t p0 = g.cls[k].pos0, p1 = p0 + ccount[k];
-            for (uint64_t w0 = p0; w0 < p1; w0 += SG_SORT_WINDOW) {
-                const uint64_t w1 = std::min<uint64_t>(p1, w0 + SG_SORT_WINDOW);
+            for (uint64_t w0 = p0; w0 < p1; w0 += SW) {
+                const uint64_t w1 = std::min<uint64_t>(p1, w0 + SW);
                 uint32_t hist[33] = {0};
                 for (uint64_t p = w0; p < w1; ++p) hist[g.row_ptr[g.orig[p] + 1] - g.row_ptr[g.orig[p]] + 1]++;
                 for (int d = 0; d < 32; ++d) hist[d + 1] += hist[d];
@@ -213,6 +214,7 @@ bool sg_build_vb_graph(uint64_t N, double c, uint64_t seed, VBHostGraph &g)
     const uint64_t entries = 32ull * g.slice_ptr[nslices];
     g.col.resize(entries); g.eid.assign(entries, SG_NONE);
     g.entry_of_edge.assign(M, 0);
+    const bool sort_rows = std::getenv("SG_VB_ROWS") == nullptr || std::strcmp(std::getenv("SG_VB_ROWS"), "edge") != 0;   // measurement knob
     for (uint64_t s = 0; s < nslices; ++s) {
         const uint64_t base = 32ull * g.slice_ptr[s];
         const uint32_t D = g.slice_ptr[s + 1] - g.slice_ptr[s];
@@ -220,12 +222,19 @@ bool sg_build_vb_graph(uint64_t N, double c, uint64_t seed, VBHostGraph &g)
             const uint64_t p = 32 * s + j;
             const uint32_t i = g.orig[p];
             const uint32_t d = g.deg[p];
+            // a row lists its neighbours by ascending position (= by class, then by BFS index): the 32 sites of a
+            // slice are close in BFS index, so their k-th neighbours tend to share 128-byte lines
+            uint64_t key[32];
+            if (i != SG_NONE) {
+                const uint64_t r0 = g.row_ptr[i];
+                for (uint32_t q = 0; q < d; ++q) key[q] = (uint64_t)g.pos[g.adj[r0 + q]] << 32 | g.adj_e[r0 + q];
+                if (sort_rows) std::sort(key, key + d);
+            }
             for (uint32_t q = 0; q < D; ++q) {
                 const uint64_t ent = base + 32ull * q + j;
                 if (i != SG_NONE && q < d) {
-                    const uint64_t r0 = g.row_ptr[i];
-                    g.col[ent] = g.pos[g.adj[r0 + q]];
-                    const uint32_t e = g.adj_e[r0 + q];
+                    g.col[ent] = (uint32_t)(key[q] >> 32);
+                    const uint32_t e = (uint32_t)key[q];
                     g.eid[ent] = e;
                     if (g.eu[e] == i) g.entry_of_edge[e] = (uint32_t)ent;
                 } else {

@@ -31,7 +31,7 @@ Philox4 sg_philox_host(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint3
 // n_words plus w, of the coupling array.  Entries beyond a site's degree (and all entries of padding positions)
 // point at the site's own position with coupling word 0.
 constexpr uint32_t SG_NONE = 0xFFFFFFFFu;
-constexpr uint32_t SG_SORT_WINDOW = 4096;
+constexpr uint32_t SG_SORT_WINDOW = 16384;
 
 struct VBClass {
     uint64_t pos0;     // first position of the class (multiple of 32)

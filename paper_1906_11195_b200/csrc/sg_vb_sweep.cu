@@ -76,6 +76,13 @@ k_vb_sweep(uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, const ui
     uint32_t nb[4];
     uint64_t jw[4];
     load_chunk(0, nb, jw);
+    // r = x_{w&3} of P(site, w>>2, sweep, tag 0): the ten Philox rounds run while the row loads are in flight
+    uint32_t x[4];
+    philox4x32_10(site, w >> 2, sweep_lo, sweep_hi, k0, k1, x);
+    const uint32_t r = (LOGW == 0) ? x[0] : ((w & 2u) ? ((w & 1u) ? x[3] : x[2]) : ((w & 1u) ? x[1] : x[0]));
+    // thr[k] is non-increasing in k, so r < thr[kk] <=> kk <= kall := #{k >= 1 : r < thr[k]} (thr[k] = 0 beyond dmax)
+    uint32_t kall = 0;
+    while (kall < 31u && (uint64_t)r < __ldg(thr + kall + 1)) ++kall;
     // Everything above reads arrays that no kernel writes.  The launch is a programmatic dependent launch: this
     // grid's CTAs start while the previous colour class is still draining and wait here, before the first spin
     // word is read, until that grid has completed and its writes are visible.
@@ -115,14 +122,8 @@ k_vb_sweep(uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, const ui
         }
     }
 
-    // r = x_{w&3} of P(site, w>>2, sweep, tag 0)
-    uint32_t x[4];
-    philox4x32_10(site, w >> 2, sweep_lo, sweep_hi, k0, k1, x);
-    const uint32_t r = (LOGW == 0) ? x[0] : ((w & 2u) ? ((w & 1u) ? x[3] : x[2]) : ((w & 1u) ? x[1] : x[0]));
-    // thr[k] is non-increasing in k, so r < thr[kk] <=> kk <= kstar := #{k >= 1 : r < thr[k]};
     // flip <=> kk = d - 2u <= kstar <=> u >= ceil((d - kstar)/2)
-    uint32_t kstar = 0;
-    while (kstar < d && (uint64_t)r < __ldg(thr + kstar + 1)) ++kstar;
+    const uint32_t kstar = min(kall, d);
     const uint32_t umin = (d - kstar + 1u) >> 1;
     uint64_t gt = 0, eq = ~0ull;
     const uint64_t pl[5] = {p0, p1, p2, p3, p4};
