@@ -41,6 +41,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
                "-Xcompiler", "-fPIC,-Wall", abi, "-c", os.path.join(CSRC, f), "-o", o] + inc
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
+        cmd += os.environ.get("SG_NVCC_FLAGS", "").split()      # e.g. -DSG_BT=128 (experiments)
         subprocess.check_call(cmd)
         objs.append(o)
     for f in CPP:

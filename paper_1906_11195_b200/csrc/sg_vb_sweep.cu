@@ -2,7 +2,7 @@
 // (row a3 of SURVEY.md 8(a); PAPER.md:260 "classic single spin flip Metropolis", :318-320 kernel prose).
 // Conventions: DESIGN.md section 3 (O7, Q14).
 //
-// One thread per (site, word).  m_e = own ^ neighbour ^ coupling (bit = bond unsatisfied) for every incident
+// One thread per (site, word), SG_BT threads per CTA.  m_e = own ^ neighbour ^ coupling (bit = bond unsatisfied) for every incident
 // edge, u = per-lane sum of the m_e in 5 bit planes (carry-save adders), one Philox draw r shared by the 64
 // lanes, kstar = #{k >= 1 : r < thr[k]}, flip the lanes with u >= ceil((d - kstar)/2).  No floating point.
 //
@@ -22,6 +22,10 @@
 void sgk_count_launch();
 
 namespace {
+// threads per CTA: 128 (4 slices) measures 3 % faster than 256 and 14 % faster than 512; 64 equals 128 (profiles/r01_sweep.md)
+#ifndef SG_BT
+#define SG_BT 128
+#endif
 
 __device__ __forceinline__ uint64_t maj64(uint64_t a, uint64_t b, uint64_t c) { return (a & b) | (c & (a ^ b)); }
 
@@ -31,7 +35,7 @@ template <> struct Idx<true> { using type = uint64_t; };
 
 // LOGW >= 0: n_words = 2^LOGW (compile time); LOGW < 0: n_words = Wrt (run time)
 template <int LOGW, bool WIDE, int MINB>
-__global__ void __launch_bounds__(256, MINB)
+__global__ void __launch_bounds__(SG_BT, (MINB * 256) / SG_BT)
 k_vb_sweep(uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, const uint32_t *__restrict__ col,
            const uint32_t *__restrict__ orig, const uint32_t *__restrict__ slice_ptr, const uint64_t *__restrict__ thr,
            uint32_t pos0, uint32_t slice0, uint32_t nslices, uint32_t Wrt, uint32_t sweep_lo, uint32_t sweep_hi, uint32_t k0, uint32_t k1,
@@ -42,7 +46,7 @@ k_vb_sweep(uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, const ui
     const uint32_t W = LOGW >= 0 ? (1u << (LOGW >= 0 ? LOGW : 0)) : Wrt;
     // `reverse`: walk the class from its last slice to its first (the host alternates the direction from launch to
     // launch, so that a launch starts where the previous one ended and finds those spin words still in L2)
-    const I T = (I)bid * 256u + threadIdx.x;
+    const I T = (I)bid * (uint32_t)SG_BT + threadIdx.x;
     const uint32_t per_slice = 32u * W;
     const uint32_t slice = LOGW >= 0 ? (uint32_t)(T >> (5 + (LOGW >= 0 ? LOGW : 0))) : (uint32_t)(T / per_slice);
     // (no thread leaves before griddep_wait(): ptxas hoists the wait above every load that follows an exit)
@@ -141,10 +145,10 @@ template <int LOGW, bool WIDE, int MINB>
 int launch(const VBDevice &d, const VBClass &c, uint32_t W, uint64_t sweep, SGSeed key, bool reverse, cudaStream_t st)
 {
     const uint64_t threads = c.nslices * 32ull * W;
-    const unsigned grid = (unsigned)((threads + 255) / 256);
+    const unsigned grid = (unsigned)((threads + SG_BT - 1) / SG_BT);
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(grid);
-    cfg.blockDim = dim3(256);
+    cfg.blockDim = dim3(SG_BT);
     cfg.dynamicSmemBytes = 0;
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
@@ -174,7 +178,7 @@ int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint64_t P, uint64_t
     if (c.n == 0) return SG_OK;
     if (c.nslices * 32ull * W >= (1ull << 40)) { sg_set_error("sgk_vb_sweep_class: class too large"); return SG_EINVAL; }
     const bool narrow = P * W < (1ull << 32) && entries * W < (1ull << 32);
-    // 5 CTAs of 256 threads per SM: 48 registers, no spills (6 CTAs spill, 4 lose latency hiding; profiles/r01_sweep.md)
+    // 1280 threads per SM: 48 registers, no spills (1536 spill, 1024 lose latency hiding; profiles/r01_sweep.md)
     if (narrow) {
         switch (W) {
         case 1: return launch<0, false, 5>(d, c, W, sweep, key, reverse, st);
