@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "sg_oracle.c")
 _LIB = os.path.join(_HERE, "liboracle.so")
 
-VB, SK = 0, 1
+VB, SK, RRBG = 0, 1, 2   # RRBG: the VB Hamiltonian on a random regular bipartite graph of degree 4
 MAX_SLOTS = 64
 
 

@@ -20,6 +20,8 @@
  *     initial spins
  *   - C(t,t') = (1/N) sum_i s_i(t) s_i(t')
  *   - energy and correlations are the observables
+ *   - model 2 (RRBG): the same Hamiltonian on a bipartite random regular graph of
+ *     degree 4, the paper's own ensemble
  *
  * Representation: spins are UNPACKED +-1 int8, one per (site, lane), in the
  * original site labels; every lane is updated on its own with explicit
@@ -41,6 +43,7 @@
 
 #define OR_VB 0
 #define OR_SK 1
+#define OR_RRBG 2   /* VB Hamiltonian on a random regular bipartite graph of degree 4 */
 #define OR_MAX_SLOTS 64
 
 typedef struct or_sim {
@@ -205,13 +208,60 @@ static void draw_initial_spins(or_sim *h)
 or_sim *or_create(int model, uint64_t N, double c, double T, uint64_t seed, uint32_t n_words)
 {
     if (N < 2 || N >= (1ull << 32) || n_words == 0) return NULL;
-    if (model != OR_VB && model != OR_SK) return NULL;
+    if (model != OR_VB && model != OR_SK && model != OR_RRBG) return NULL;
+    if (model == OR_RRBG && (N < 8 || (N & 1))) return NULL;   /* two halves of N/2 >= 4 vertices */
     if (!(T >= 0.0)) return NULL;
     or_sim *h = (or_sim *)calloc(1, sizeof(or_sim));
     h->model = model; h->N = N; h->W = n_words; h->T = T; h->seed = seed; h->sweep = 0;
     if (alloc_state(h)) { or_destroy(h); return NULL; }
 
-    if (model == OR_VB) {
+    if (model == OR_RRBG) {
+        /* O2b: random regular bipartite graph of degree 4, "all of them are in the same half of the lattice"
+         * (PAPER.md:318), as the union of four permutations of one half onto the other without a repeated pair.
+         * Halves A = {0..H-1}, B = {H..N-1}, H = N/2.  Permutation a = 0..3: attempts t = 0,1,2,... (one global
+         * counter); an attempt is a Fisher-Yates shuffle of the identity, for i = H-1 down to 1:
+         * j = (x*(i+1)) >> 32 with x = word n&3 of P(n>>2, t, 0, tag 4), n = H-1-i, swap(perm[i], perm[j]);
+         * it is accepted if perm[i] differs from every earlier accepted permutation at every i.
+         * Edge e = a*H + i joins i and H + perm_a[i]. */
+        const uint64_t H = N / 2;
+        h->M = 4 * H;
+        h->eu = (uint32_t *)malloc((h->M + 1) * sizeof(uint32_t));
+        h->ev = (uint32_t *)malloc((h->M + 1) * sizeof(uint32_t));
+        uint32_t *perm = (uint32_t *)malloc(H * sizeof(uint32_t));
+        uint64_t t = 0;
+        for (uint32_t a = 0; a < 4; ++a) {
+            for (;; ++t) {
+                for (uint64_t i = 0; i < H; ++i) perm[i] = (uint32_t)i;
+                uint32_t x[4] = {0, 0, 0, 0};
+                for (uint64_t i = H - 1; i >= 1; --i) {
+                    const uint64_t n = H - 1 - i;
+                    if ((n & 3) == 0) P(h, (uint32_t)(n >> 2), (uint32_t)t, 0, 4, x);
+                    const uint64_t j = ((uint64_t)x[n & 3] * (i + 1)) >> 32;
+                    const uint32_t tmp = perm[i]; perm[i] = perm[j]; perm[j] = tmp;
+                }
+                int clash = 0;
+                for (uint32_t b = 0; b < a && !clash; ++b)
+                    for (uint64_t i = 0; i < H; ++i)
+                        if (h->ev[(uint64_t)b * H + i] == (uint32_t)(H + perm[i])) { clash = 1; break; }
+                if (!clash) { ++t; break; }
+            }
+            for (uint64_t i = 0; i < H; ++i) {
+                h->eu[(uint64_t)a * H + i] = (uint32_t)i;
+                h->ev[(uint64_t)a * H + i] = (uint32_t)(H + perm[i]);
+            }
+        }
+        free(perm);
+        h->model = OR_VB;   /* from here on: the VB Hamiltonian (Eq. 3) on this edge list */
+        if (build_csr_colour_thr(h)) { or_destroy(h); return NULL; }
+        const uint64_t M = h->M;
+        h->kappa = (uint64_t *)malloc((M * h->W + 1) * sizeof(uint64_t));
+        for (uint64_t f = 0; f < M; ++f)
+            for (uint32_t w = 0; w < h->W; ++w) {
+                uint32_t x[4];
+                P(h, (uint32_t)f, w, 0, 2, x);
+                h->kappa[f * h->W + w] = (uint64_t)x[0] | ((uint64_t)x[1] << 32);
+            }
+    } else if (model == OR_VB) {
         /* O2: G(N, M), M = floor(c N / 2 + 0.5); attempts a = 0,1,2,... */
         if (!(c >= 0.0)) { or_destroy(h); return NULL; }
         double pairs = 0.5 * (double)N * (double)(N - 1);
