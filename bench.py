@@ -38,7 +38,8 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--T", type=float, default=1.0)
-    ap.add_argument("--model", default="vb", choices=["vb", "sk"], help="sk: BASELINE.json configs[3] with --log2n 12 (absolute rate only)")
+    ap.add_argument("--model", default="vb", choices=["vb", "sk", "rrbg"],
+                    help="sk: BASELINE.json configs[3] with --log2n 12 (absolute rate only); rrbg: the paper's own ensemble (SURVEY.md 8(f) rank 1), use --T 1.2149")
     ap.add_argument("--log2n", type=int, default=24)
     ap.add_argument("--n-words", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -160,7 +161,7 @@ def run_ours(args):
     t0 = time.perf_counter()
     from paper_1906_11195_b200.workloads import Workload, shard
 
-    model = sg.SG_MODEL_SK if args.model == "sk" else sg.SG_MODEL_VB
+    model = {"vb": sg.SG_MODEL_VB, "sk": sg.SG_MODEL_SK, "rrbg": sg.SG_MODEL_RRBG}[args.model]
     wl = shard(Workload("bench", model, N, 4.0, args.T, 1, W, 0), rank, world)
     sim = sg.Sim(wl.model, wl.N, wl.c, wl.T, wl.seed, wl.n_words)
     create_s = time.perf_counter() - t0
@@ -244,6 +245,7 @@ def run_ours(args):
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "u64", "data": "synthetic",
         "config": {"workload": (f"VB N=2^{args.log2n} c=4 W={W} T={args.T} seed=1+rank (BASELINE.json configs[2])" if args.model == "vb"
+                                else f"RRBG degree 4 N=2^{args.log2n} W={W} T={args.T} seed=1+rank (the paper's ensemble, PAPER.md:260; not the headline workload)" if args.model == "rrbg"
                                 else f"SK N=2^{args.log2n} W={W} T={args.T} seed=1+rank (BASELINE.json configs[3]; dependency-latency bound, roofline fields not meaningful)"),
                    "step": f"sg_sweep({SWEEPS_PER_STEP}) + sg_snapshot + sg_correlation + sg_energy",
                    "l2": "inputs larger than L2: every sweep streams 777 MiB of couplings+indices+labels and reads/writes the 128 MiB spin array (L2 126 MiB); no flush needed",
@@ -266,7 +268,7 @@ def run_ours(args):
         out["roofline"] = {"bound": "latency", "kernel": "k_sk_sweep", "achieved": None, "peak": None, "unit": None, "frac": None, "traffic": None,
                            "note": "sequential sweep of one instance per CTA (PAPER.md:233): dependency-latency bound, absolute rate only",
                            "sweep_ms": sweep_ms / (SWEEPS_PER_STEP * args.steps)}
-    if not args.no_cpu_baseline and args.model == "vb":
+    if not args.no_cpu_baseline and args.model == "vb":   # the headline ensemble only
         v, dt, n = cpu_sample(args, 2)
         out["cpu_baseline"] = {"value": v, "unit": "spin updates/s", "cores": 1, "kind": "oracle", "host_cores": os.cpu_count(),
                                "sample": f"same recipe at N=2^{n.bit_length() - 1}, 2 oracle sweeps, {dt:.1f} s"}

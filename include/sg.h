@@ -29,7 +29,7 @@ extern "C" {
 
 typedef struct sg_sim sg_sim; /* opaque; owns every device and host buffer of one simulation */
 
-enum { SG_MODEL_VB = 0, SG_MODEL_SK = 1 };
+enum { SG_MODEL_VB = 0, SG_MODEL_SK = 1, SG_MODEL_RRBG = 2 };
 enum { SG_OK = 0, SG_EINVAL = -1, SG_ENOMEM = -2, SG_ECUDA = -3, SG_ESLOT = -4 };
 #define SG_MAX_SLOTS 64
 
@@ -40,6 +40,10 @@ enum { SG_OK = 0, SG_EINVAL = -1, SG_ENOMEM = -2, SG_ECUDA = -3, SG_ESLOT = -4 }
  *                        M = floor(c*N/2 + 0.5), self-loops and multi-edges rejected (O2);
  *           SG_MODEL_SK: Sherrington-Kirkpatrick model (Eq. 1) with binary couplings
  *                        +-1/sqrt(N); c is ignored.
+ *           SG_MODEL_RRBG: the Viana-Bray Hamiltonian on the paper's own graph ensemble, a random regular
+ *                        bipartite graph of degree 4: halves {0..N/2-1} and {N/2..N-1},
+ *                        four clash-free random permutations of one half onto the other (O2b), hence
+ *                        exactly two colour classes; N even and >= 8; c is ignored.
  *   N       number of sites, 2 <= N < 2^31 (SK: N <= 32768 so that int16 local fields are exact).
  *   c       mean degree (VB), c >= 0 and M <= N(N-1)/2.
  *   T       temperature, 0 <= T <= +inf (T = 0 and T = inf are legal).
@@ -145,7 +149,7 @@ void sg_host_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t
  * No output depends on this relabelling: the Philox counter uses the original label (Q15).
  */
 typedef struct sg_host_graph sg_host_graph;
-sg_host_graph *sg_host_graph_create(uint64_t N, double c, uint64_t seed);   /* NULL on bad arguments */
+sg_host_graph *sg_host_graph_create(int model, uint64_t N, double c, uint64_t seed);   /* model: SG_MODEL_VB or SG_MODEL_RRBG; NULL on bad arguments */
 void sg_host_graph_destroy(sg_host_graph *g);
 /* info HOST 8 uint64: M, K (colours), dmax, entries, nslices, N, P (positions incl. padding), sort_window */
 int sg_host_graph_info(const sg_host_graph *g, uint64_t *info);

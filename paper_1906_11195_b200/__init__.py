@@ -4,6 +4,7 @@ Thin Python binding over the C-ABI of include/sg.h (libsg.so).  The binding mars
 arguments only: every step of the path runs in the library's CUDA kernels.
 """
 from .binding import (  # noqa: F401
+    SG_MODEL_RRBG,
     SG_MODEL_SK,
     SG_MODEL_VB,
     SGError,

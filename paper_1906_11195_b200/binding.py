@@ -9,7 +9,7 @@ import os
 
 import numpy as np
 
-SG_MODEL_VB, SG_MODEL_SK = 0, 1
+SG_MODEL_VB, SG_MODEL_SK, SG_MODEL_RRBG = 0, 1, 2
 SG_OK, SG_EINVAL, SG_ENOMEM, SG_ECUDA, SG_ESLOT = 0, -1, -2, -3, -4
 SG_MAX_SLOTS = 64
 
@@ -39,7 +39,7 @@ SYMBOLS = {
     "sg_get_thresholds": (C.c_int, [_vp, _vp, _u64]),
     "sg_kernel_launches": (_u64, []),
     "sg_host_philox": (None, [_u32] * 6 + [_vp]),
-    "sg_host_graph_create": (_vp, [_u64, _dbl, _u64]),
+    "sg_host_graph_create": (_vp, [C.c_int, _u64, _dbl, _u64]),
     "sg_host_graph_destroy": (None, [_vp]),
     "sg_host_graph_info": (C.c_int, [_vp, _vp]),
     "sg_host_graph_get": (C.c_int, [_vp] * 12),
@@ -229,10 +229,10 @@ def host_philox(c0, c1, c2, c3, k0, k1) -> np.ndarray:
     return out
 
 
-def host_graph(N: int, c: float, seed: int) -> dict:
+def host_graph(N: int, c: float, seed: int, model: int = SG_MODEL_VB) -> dict:
     """The device layout of a VB instance, built by the library's host generator only."""
     L = load_library()
-    g = L.sg_host_graph_create(int(N), float(c), int(seed))
+    g = L.sg_host_graph_create(int(model), int(N), float(c), int(seed))
     if not g:
         raise SGError(SG_EINVAL, _err())
     try:

@@ -33,7 +33,7 @@ void destroy_impl(sg_sim *h)
 int create_vb(sg_sim *h)
 {
     cudaStream_t st = sgx_stream();
-    if (!sg_build_vb_graph(h->N, h->c, h->seed, h->g)) return SG_EINVAL;
+    if (!sg_build_vb_graph(h->graph_model, h->N, h->c, h->seed, h->g)) return SG_EINVAL;
     VBHostGraph &g = h->g;
     h->M = g.M;
     const uint64_t W = h->W, P = g.P;
@@ -74,7 +74,7 @@ int create_vb(sg_sim *h)
 extern "C" sg_sim *sg_create(int model, uint64_t N, double c, double T, uint64_t seed, uint32_t n_words)
 {
     g_err.clear();
-    if (model != SG_MODEL_VB && model != SG_MODEL_SK) { sg_set_error("sg_create: unknown model"); return nullptr; }
+    if (model != SG_MODEL_VB && model != SG_MODEL_SK && model != SG_MODEL_RRBG) { sg_set_error("sg_create: unknown model"); return nullptr; }
     if (N < 2 || N >= (1ull << 31)) { sg_set_error("sg_create: N must satisfy 2 <= N < 2^31"); return nullptr; }
     if (n_words == 0) { sg_set_error("sg_create: n_words must be >= 1"); return nullptr; }
     if (!(T >= 0.0)) { sg_set_error("sg_create: T must be >= 0 (T = inf allowed)"); return nullptr; }
@@ -83,6 +83,9 @@ extern "C" sg_sim *sg_create(int model, uint64_t N, double c, double T, uint64_t
     if (!sgx_device_ok(&why)) { sg_set_error("sg_create: " + why); return nullptr; }
     sg_sim *h = new (std::nothrow) sg_sim();
     if (!h) { sg_set_error("sg_create: out of host memory"); return nullptr; }
+    // RRBG is the VB Hamiltonian on another graph ensemble: only the host generator tells them apart
+    h->graph_model = model;
+    if (model == SG_MODEL_RRBG) model = SG_MODEL_VB;
     h->model = model; h->N = N; h->W = n_words; h->c = c; h->T = T; h->seed = seed;
     h->key = SGSeed{(uint32_t)seed, (uint32_t)(seed >> 32)};
     int rc;

@@ -81,7 +81,46 @@ struct PairSet {
 };
 }  // namespace
 
-bool sg_build_vb_graph(uint64_t N, double c, uint64_t seed, VBHostGraph &g)
+// O2b: random regular bipartite graph of degree 4 as the union of four permutations of
+// half A = {0..H-1} onto half B = {H..N-1}, H = N/2, without a repeated pair.  Permutation a = 0..3: attempts
+// t = 0,1,2,... (one counter over all four); an attempt is a Fisher-Yates shuffle of the identity, for i = H-1 down
+// to 1: j = (x*(i+1)) >> 32 with x = word n&3 of P(n>>2, t, 0, tag 4), n = H-1-i, swap(perm[i], perm[j]); it is
+// accepted if it differs from every earlier accepted permutation at every i.  Edge e = a*H + i joins i and H + perm_a[i].
+static bool build_rrbg_edges(uint64_t N, uint64_t seed, VBHostGraph &g)
+{
+    if (N < 8 || (N & 1)) { sg_set_error("sg_create: the RRBG model needs an even N >= 8"); return false; }
+    const uint64_t H = N / 2;
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    g.N = N; g.M = 4 * H;
+    g.eu.resize(g.M); g.ev.resize(g.M);
+    std::vector<uint32_t> perm(H);
+    uint64_t t = 0;
+    for (uint32_t a = 0; a < 4; ++a) {
+        for (;; ++t) {
+            std::iota(perm.begin(), perm.end(), 0u);
+            Philox4 x{{0, 0, 0, 0}};
+            for (uint64_t i = H - 1; i >= 1; --i) {
+                const uint64_t n = H - 1 - i;
+                if ((n & 3) == 0) x = sg_philox_host((uint32_t)(n >> 2), (uint32_t)t, 0u, 4u << 24, k0, k1);
+                const uint64_t j = ((uint64_t)x.x[n & 3] * (i + 1)) >> 32;
+                std::swap(perm[i], perm[j]);
+            }
+            bool clash = false;
+            for (uint32_t b = 0; b < a && !clash; ++b)
+                for (uint64_t i = 0; i < H; ++i)
+                    if (g.ev[(uint64_t)b * H + i] == (uint32_t)(H + perm[i])) { clash = true; break; }
+            if (!clash) { ++t; break; }
+        }
+        for (uint64_t i = 0; i < H; ++i) {
+            g.eu[(uint64_t)a * H + i] = (uint32_t)i;
+            g.ev[(uint64_t)a * H + i] = (uint32_t)(H + perm[i]);
+        }
+    }
+    return true;
+}
+
+// O2: Erdos-Renyi G(N, M), M = floor(c N / 2 + 0.5), self-loops and repeated pairs rejected
+static bool build_er_edges(uint64_t N, double c, uint64_t seed, VBHostGraph &g)
 {
     if (!(c >= 0.0) || !std::isfinite(c)) { sg_set_error("sg_create: c must be finite and >= 0"); return false; }
     const double pairs = 0.5 * (double)N * (double)(N - 1);
@@ -92,19 +131,24 @@ bool sg_build_vb_graph(uint64_t N, double c, uint64_t seed, VBHostGraph &g)
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     g.N = N; g.M = M;
     g.eu.resize(M); g.ev.resize(M);
-    {
-        PairSet seen(M);
-        uint64_t e = 0;
-        for (uint64_t a = 0; e < M; ++a) {
-            const Philox4 x = sg_philox_host((uint32_t)a, (uint32_t)(a >> 32), 0u, 3u << 24, k0, k1);
-            const uint32_t u = (uint32_t)(((uint64_t)x.x[0] * N) >> 32);
-            const uint32_t v = (uint32_t)(((uint64_t)x.x[1] * N) >> 32);
-            if (u == v) continue;
-            const uint64_t key = u < v ? ((uint64_t)u << 32 | v) : ((uint64_t)v << 32 | u);
-            if (!seen.insert(key)) continue;
-            g.eu[e] = u; g.ev[e] = v; ++e;
-        }
+    PairSet seen(M);
+    uint64_t e = 0;
+    for (uint64_t a = 0; e < M; ++a) {
+        const Philox4 x = sg_philox_host((uint32_t)a, (uint32_t)(a >> 32), 0u, 3u << 24, k0, k1);
+        const uint32_t u = (uint32_t)(((uint64_t)x.x[0] * N) >> 32);
+        const uint32_t v = (uint32_t)(((uint64_t)x.x[1] * N) >> 32);
+        if (u == v) continue;
+        const uint64_t key = u < v ? ((uint64_t)u << 32 | v) : ((uint64_t)v << 32 | u);
+        if (!seen.insert(key)) continue;
+        g.eu[e] = u; g.ev[e] = v; ++e;
     }
+    return true;
+}
+
+bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, VBHostGraph &g)
+{
+    if (model == SG_MODEL_RRBG ? !build_rrbg_edges(N, seed, g) : !build_er_edges(N, c, seed, g)) return false;
+    const uint64_t M = g.M;
     // CSR in original labels, rows in increasing edge id
     g.row_ptr.assign(N + 1, 0);
     for (uint64_t e = 0; e < M; ++e) { g.row_ptr[g.eu[e] + 1]++; g.row_ptr[g.ev[e] + 1]++; }
@@ -255,11 +299,12 @@ extern "C" void sg_host_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c
     for (int q = 0; q < 4; ++q) out[q] = x.x[q];
 }
 
-extern "C" sg_host_graph *sg_host_graph_create(uint64_t N, double c, uint64_t seed)
+extern "C" sg_host_graph *sg_host_graph_create(int model, uint64_t N, double c, uint64_t seed)
 {
+    if (model != SG_MODEL_VB && model != SG_MODEL_RRBG) { sg_set_error("sg_host_graph_create: graph model required"); return nullptr; }
     if (N < 2 || N >= (1ull << 32)) { sg_set_error("sg_host_graph_create: N must satisfy 2 <= N < 2^32"); return nullptr; }
     sg_host_graph *h = new sg_host_graph();
-    if (!sg_build_vb_graph(N, c, seed, h->g)) { delete h; return nullptr; }
+    if (!sg_build_vb_graph(model, N, c, seed, h->g)) { delete h; return nullptr; }
     return h;
 }
 

@@ -60,7 +60,7 @@ struct VBHostGraph {
 };
 
 // Builds everything above.  Returns false and sets the error string on bad arguments.
-bool sg_build_vb_graph(uint64_t N, double c, uint64_t seed, VBHostGraph &g);
+bool sg_build_vb_graph(int model /* SG_MODEL_VB or SG_MODEL_RRBG */, uint64_t N, double c, uint64_t seed, VBHostGraph &g);
 
 std::vector<uint64_t> sg_vb_thresholds(double T, uint32_t dmax);   // thr[0..dmax], thr[0]=0
 std::vector<uint64_t> sg_sk_thresholds(double T, uint64_t N);      // thr[0..N-1]

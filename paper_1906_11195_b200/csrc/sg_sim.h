@@ -8,7 +8,8 @@
 #include "sg_internal.h"
 
 struct sg_sim {
-    int model = SG_MODEL_VB;
+    int model = SG_MODEL_VB;                 // SG_MODEL_VB (also for RRBG instances) or SG_MODEL_SK
+    int graph_model = SG_MODEL_VB;           // the graph ensemble: SG_MODEL_VB (Erdos-Renyi) or SG_MODEL_RRBG
     uint64_t N = 0, M = 0;
     uint32_t W = 0;
     double c = 0, T = 0;

@@ -9,7 +9,7 @@ from __future__ import annotations
 
 from dataclasses import dataclass
 
-VB, SK = 0, 1
+VB, SK, RRBG = 0, 1, 2
 
 
 @dataclass(frozen=True)
@@ -29,6 +29,11 @@ CFG1 = Workload("cfg1_vb_n1024", VB, 1 << 10, 4.0, 1.0, 1, 1, 1 << 10)
 CFG2 = Workload("cfg2_vb_n2^20_w4", VB, 1 << 20, 4.0, 1.0, 1, 4, 1 << 14)
 CFG3 = [Workload(f"cfg3_vb_n2^24_T{T}", VB, 1 << 24, 4.0, T, 1, 1, 1 << 12) for T in (0.6, 1.0, 1.4)]
 CFG4 = Workload("cfg4_sk_n4096", SK, 1 << 12, 0.0, 0.6, 1, 1, 1 << 12)
+
+
+# The paper's own workload: RRBG degree 4, T = 0.8 Tc = 0.8 / atanh(1/sqrt(3))
+T_PAPER = 0.8 / 0.6584789484624083      # atanh(1/sqrt(3)) = 0.658478948...
+PAPER_RRBG = Workload("paper_rrbg_n2^24", RRBG, 1 << 24, 0.0, T_PAPER, 1, 1, 1 << 12)
 
 
 def cfg5():

@@ -273,3 +273,43 @@ def test_largest_size_properties(sg, T):
         assert np.all(D1 <= N) and np.all(D1 > 0)
         # per-lane energy of a random +-J configuration is ~0 +- sqrt(M); a T=0 quench lowers it by O(N)
         assert np.all(E3 < -0.5 * N)
+
+
+@pytest.mark.parametrize("N,T,seed,W", [(1024, 1.2149, 1, 1), (8, 1.0, 2, 1), (4102, 0.6, 3, 2), (1 << 16, 1.2149, 4, 1)])
+def test_rrbg_matches_oracle(sg, oracle_mod, N, T, seed, W):
+    """SG_MODEL_RRBG: the paper's own ensemble (random regular bipartite graph of degree 4, two colour classes)."""
+    g = sg.Sim(sg.SG_MODEL_RRBG, N, 0.0, T, seed, W)
+    o = oracle_mod.Oracle(oracle_mod.RRBG, N, 0.0, T, seed, W)
+    assert g.M == o.M == 2 * N and g.n_colours == o.n_colours == 2 and g.max_degree == 4
+    assert np.array_equal(g.edges(), o.edges())
+    assert np.array_equal(g.couplings(), o.couplings())
+    _assert_same_state(g, o)
+    g.snapshot(0); o.snapshot(0)
+    for _ in range(5):
+        g.sweep(2)
+        o.sweep(2)
+        _assert_same_state(g, o)
+        assert np.array_equal(g.energy(), o.energy())
+        assert np.array_equal(g.correlation(0), o.correlation(0))
+
+
+def test_rrbg_full_size_late_sweep(sg, oracle_mod):
+    """The paper's workload at N = 2^24 (W = 1, T = 0.8 Tc): one late sweep against the oracle, element by element."""
+    from paper_1906_11195_b200.workloads import PAPER_RRBG as w
+
+    g = sg.Sim(w.model, w.N, w.c, w.T, w.seed, w.n_words)
+    o = oracle_mod.Oracle(oracle_mod.RRBG, w.N, w.c, w.T, w.seed, w.n_words)
+    assert np.array_equal(g.spins(), o.spins())
+    g.sweep(30)
+    before = g.spins()
+    E_before = g.energy()
+    g.snapshot(0)
+    o.set_spins(before)
+    o.set_sweep_count(30)
+    dE0 = o.accumulated_dE().copy()
+    g.sweep(1)
+    o.sweep(1)
+    after = g.spins()
+    assert np.array_equal(after, o.spins())
+    assert np.array_equal(g.energy() - E_before, o.accumulated_dE() - dE0)
+    assert np.array_equal(g.correlation(0), _lane_counts(before ^ after))

@@ -46,7 +46,7 @@ def test_no_cpu_fallback(sg):
 def test_bad_arguments_are_rejected_before_touching_the_gpu(sg):
     for args in [(7, 100, 4.0, 1.0, 1, 1), (0, 1, 4.0, 1.0, 1, 1), (0, 100, 4.0, 1.0, 1, 0),
                  (0, 100, 4.0, -0.5, 1, 1), (0, 100, 4.0, float("nan"), 1, 1), (1, 40000, 0.0, 1.0, 1, 1),
-                 (0, 1 << 31, 4.0, 1.0, 1, 1)]:
+                 (0, 1 << 31, 4.0, 1.0, 1, 1), (2, 1001, 0.0, 1.0, 1, 1), (2, 6, 0.0, 1.0, 1, 1)]:
         with pytest.raises(sg.SGError):
             sg.Sim(*args)
 
@@ -61,12 +61,14 @@ def test_host_philox_known_answers(sg):
         assert list(binding.host_philox(*v[:6])) == v[6:]
 
 
-@pytest.mark.parametrize("N,c,seed", [(1024, 4.0, 1), (5000, 4.0, 77), (333, 2.5, 3), (64, 7.0, 5), (100, 0.0, 1)])
-def test_host_generator_matches_oracle_and_layout_is_consistent(sg, oracle_mod, N, c, seed):
+@pytest.mark.parametrize("model,N,c,seed", [(0, 1024, 4.0, 1), (0, 5000, 4.0, 77), (0, 333, 2.5, 3), (0, 64, 7.0, 5), (0, 100, 0.0, 1),
+                                            (2, 8, 0.0, 1), (2, 1024, 0.0, 2), (2, 4102, 0.0, 3)])
+def test_host_generator_matches_oracle_and_layout_is_consistent(sg, oracle_mod, model, N, c, seed):
+    """model 0: Erdos-Renyi (O2); model 2: random regular bipartite graph of degree 4 (O2b)."""
     from paper_1906_11195_b200 import binding
 
-    g = binding.host_graph(N, c, seed)
-    o = oracle_mod.Oracle(oracle_mod.VB, N, c, 1.0, seed, 1)
+    g = binding.host_graph(N, c, seed, model)
+    o = oracle_mod.Oracle(model, N, c, 1.0, seed, 1)
     assert g["M"] == o.M and g["K"] == o.n_colours and g["dmax"] == o.max_degree
     e = o.edges()
     assert np.array_equal(g["u"], e[:, 0]) and np.array_equal(g["v"], e[:, 1])
