@@ -94,3 +94,41 @@ def shard(w: Workload, rank: int, world: int) -> Workload:
 def global_lane(w: Workload, rank: int, lane: int) -> int:
     """Index of a rank's lane in the job-wide, rank-major list of samples."""
     return rank * 64 * w.n_words + lane
+
+
+# ---- windowed protocol (SURVEY.md 8(f) rank 2; PAPER.md:95, :270) ---------------------------------------------------------
+def window_index(time: int) -> int:
+    """Index m of the minor-third logarithmic interval (t_m, t_{m+1}], t_m = 2^(m/4), that contains the integer time
+    (PAPER.md:270: "minor thirds logarithmic intervals tw + t in [t_m, t_{m+1}], with t_{m+1}/t_m = 2^{1/4}").
+    Integer-exact: m = ceil(4 log2 time) - 1 for time >= 2, found by comparing time^4 with 2^m; time 1 -> m = -1."""
+    if time < 1:
+        raise ValueError("time must be >= 1")
+    t4 = time ** 4
+    m = t4.bit_length() - 1                  # 2^m <= time^4 < 2^(m+1)
+    return m - 1 if t4 == 1 << m else m      # time^4 in (2^m, 2^(m+1)]  <=>  time in (t_m, t_{m+1}]
+
+
+def run_windowed(sim, total_sweeps: int, tws=(4, 16, 64, 256, 1024, 4096)):
+    """The paper's measurement protocol on any object with sweep/snapshot/correlation (the binding's Sim or the oracle's
+    handle): snapshot at every waiting time tw (tw = 2^2, 2^4, ..., 2^12), then after EVERY sweep count D
+    against every stored tw and add it to the bin of the total time tw + t (window_index).  Returns
+    {(tw, m): (sum of D over the bin as uint64 per lane, number of times in the bin)}: the caller's window average is
+    C = 1 - 2 * sumD / (n * N).  Exact integers; no arithmetic of the method is done here."""
+    import numpy as np
+
+    tws = [tw for tw in tws if tw <= total_sweeps]
+    slot_of = {tw: k for k, tw in enumerate(tws)}
+    out = {}
+    for time in range(1, total_sweeps + 1):
+        sim.sweep(1)
+        for tw in tws:
+            if time > tw:
+                key = (tw, window_index(time))
+                d = np.asarray(sim.correlation(slot_of[tw]), dtype=np.uint64)
+                if key in out:
+                    out[key] = (out[key][0] + d, out[key][1] + 1)
+                else:
+                    out[key] = (d.copy(), 1)
+        if time in slot_of:
+            sim.snapshot(slot_of[time])
+    return out

@@ -313,3 +313,17 @@ def test_rrbg_full_size_late_sweep(sg, oracle_mod):
     assert np.array_equal(after, o.spins())
     assert np.array_equal(g.energy() - E_before, o.accumulated_dE() - dE0)
     assert np.array_equal(g.correlation(0), _lane_counts(before ^ after))
+
+
+def test_windowed_protocol_matches_oracle(sg, oracle_mod):
+    """The paper's measurement protocol (snapshots at tw = 4, 16, 64; D against every tw after every sweep, binned in
+    minor-third intervals of tw + t) gives the same exact sums on the GPU path and on the oracle."""
+    from paper_1906_11195_b200.workloads import run_windowed
+
+    N, S = 4096, 100
+    g = sg.Sim(sg.SG_MODEL_RRBG, N, 0.0, 1.2149, 5, 2)
+    o = oracle_mod.Oracle(oracle_mod.RRBG, N, 0.0, 1.2149, 5, 2)
+    rg, ro = run_windowed(g, S), run_windowed(o, S)
+    assert rg.keys() == ro.keys() and len(rg) > 20
+    for k in rg:
+        assert rg[k][1] == ro[k][1] and np.array_equal(rg[k][0], ro[k][0]), k

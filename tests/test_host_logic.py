@@ -169,3 +169,53 @@ def test_schedule_counts():
             snapped.add(slot)
         else:
             assert slot in snapped and t > (1 << slot) and bin(t - (1 << slot)).count("1") == 1
+
+
+def test_window_index_is_the_minor_third_bin():
+    """bins (t_m, t_{m+1}] with t_m = 2^(m/4); checked against floating point away from the bin edges and
+    exactly at the edges that are integers (t = 2^k = t_{4k} belongs to bin 4k - 1)."""
+    import math
+
+    from paper_1906_11195_b200.workloads import window_index
+
+    assert window_index(1) == -1
+    for k in range(1, 40):
+        assert window_index(1 << k) == 4 * k - 1
+        if k >= 3:
+            assert window_index((1 << k) + 1) == 4 * k
+    for t in list(range(2, 5000)) + [10**6 + 7, 2**25 - 1]:
+        m = window_index(t)
+        assert 2.0 ** (m / 4) < t <= 2.0 ** ((m + 1) / 4) * (1 + 1e-12)
+    # the bins of 1..T partition the times, and bin widths grow by 2^(1/4)
+    T = 4096
+    seen = {}
+    for t in range(2, T + 1):
+        seen.setdefault(window_index(t), []).append(t)
+    assert sum(len(v) for v in seen.values()) == T - 1
+    big = [m for m in seen if m >= 40 and m + 1 in seen and max(seen[m + 1]) < T]
+    for m in big:
+        assert abs(len(seen[m + 1]) / len(seen[m]) - 2 ** 0.25) < 0.15
+
+
+def test_windowed_protocol_on_the_oracle(oracle_mod):
+    """run_windowed against a direct recomputation from stored configurations (small N, the oracle as the simulator)."""
+    from paper_1906_11195_b200.workloads import run_windowed, window_index
+
+    N, S = 512, 80
+    o = oracle_mod.Oracle(oracle_mod.RRBG, N, 0.0, 1.2149, 3, 1)
+    res = run_windowed(o, S, tws=(4, 16, 64, 256))
+    o2 = oracle_mod.Oracle(oracle_mod.RRBG, N, 0.0, 1.2149, 3, 1)
+    from tests import exact
+    states = {0: exact.unpack(o2.spins())}
+    for t in range(1, S + 1):
+        o2.sweep(1)
+        states[t] = exact.unpack(o2.spins())
+    expect = {}
+    for tw in (4, 16, 64):
+        for t in range(tw + 1, S + 1):
+            key = (tw, window_index(t))
+            d = (states[t] != states[tw]).sum(axis=0).astype(np.uint64)
+            expect[key] = (expect[key][0] + d, expect[key][1] + 1) if key in expect else (d, 1)
+    assert res.keys() == expect.keys()
+    for k in res:
+        assert res[k][1] == expect[k][1] and np.array_equal(res[k][0], expect[k][0]), k
