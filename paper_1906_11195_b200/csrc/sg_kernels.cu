@@ -236,15 +236,22 @@ k_xor_popcount(const uint64_t *__restrict__ a, const uint64_t *__restrict__ b, u
     const uint32_t w_fixed = CONTIG ? 0u : blockIdx.y;
     const uint32_t G = CONTIG ? W : 1u;
     uint32_t pending = 0;
-    for (uint64_t ch = warp; ch < nchunks; ch += nwarps) {
-        const uint64_t q = ch * 32 + lane;
-        uint64_t x = 0;
-        if (q < total) {
-            const uint64_t idx = CONTIG ? q : q * W + w_fixed;
-            x = ld_plain_u64(a + idx) ^ ld_stream_u64(b + idx, pol_stream);
+    constexpr int U = 4;                       // chunks per iteration: 2*U loads in flight per thread
+    for (uint64_t ch = warp; ch < nchunks; ch += (uint64_t)U * nwarps) {
+        uint64_t x[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const uint64_t q = (ch + (uint64_t)u * nwarps) * 32 + lane;
+            x[u] = 0;
+            if (q < total) {
+                const uint64_t idx = CONTIG ? q : q * W + w_fixed;
+                x[u] = ld_plain_u64(a + idx) ^ ld_stream_u64(b + idx, pol_stream);
+            }
         }
-        vc_add_bit<P, PT>(acc, x);
-        if (++pending == (1u << P) - 1u) {
+#pragma unroll
+        for (int u = 0; u < U; ++u) vc_add_bit<P, PT>(acc, x[u]);
+        pending += U;
+        if (pending + U > (1u << P) - 1u) {
             vc_warp_flush<PT>(acc, G, w_fixed, counts);
             vc_clear(acc);
             pending = 0;
