@@ -262,6 +262,9 @@ def run_ours(args):
     if os.path.exists(tr) and headline:      # ncu dram bytes of one sweep of exactly this workload (profiles/r01_sweep.md)
         out["roofline"]["traffic"] = json.load(open(tr)).get("dram_bytes_per_sweep")
         out["roofline"]["per"] = "sweep (the K colour-class launches): achieved, traffic and sweep_ms are per sweep"
+        out["roofline"]["dram_bytes_per_site_word"] = out["roofline"]["traffic"] / (N * W)       # ncu, BASELINE.md section 2
+        out["roofline"]["frac_104B"] = out["roofline"]["frac"] * 104.0 / 80.0                    # + indices, row pointer, label
+        out["roofline"]["philox_alu_ceiling_spin_updates_per_s"] = 5.79e11 * 64                  # profiles/r01_probes.md
     if not headline:
         out["config"]["l2"] = "not the headline workload: see DESIGN.md section 10"
     if args.model == "sk":
