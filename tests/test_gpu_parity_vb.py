@@ -207,14 +207,15 @@ def _lane_counts(x):
     return out
 
 
-def test_full_size_config3_late_sweep(sg, oracle_mod):
-    """BASELINE.json configs[2] at full size (N = 2^24, W = 1, T = 1), in the launch configuration bench.py times:
+@pytest.mark.parametrize("T", [1.0, 0.6])
+def test_full_size_config3_late_sweep(sg, oracle_mod, T):
+    """BASELINE.json configs[2] at full size (N = 2^24, W = 1, T = 1 and 0.6), in the launch configuration bench.py times:
     the GPU runs 40 sweeps, then ONE more sweep is compared element by element with the oracle started from the
     GPU's state at sweep 40 (a sweep is a pure function of (state, index), Q15), together with the
     correlation counts against a snapshot and the energy change (oracle's accumulated dE of that sweep)."""
     N, W, T0 = 1 << 24, 1, 40
-    g = sg.Sim(sg.SG_MODEL_VB, N, 4.0, 1.0, 1, W)
-    o = oracle_mod.Oracle(oracle_mod.VB, N, 4.0, 1.0, 1, W)
+    g = sg.Sim(sg.SG_MODEL_VB, N, 4.0, T, 1, W)
+    o = oracle_mod.Oracle(oracle_mod.VB, N, 4.0, T, 1, W)
     assert g.M == o.M and g.n_colours == o.n_colours and g.max_degree == o.max_degree
     assert np.array_equal(g.spins(), o.spins())                   # initial configuration
     idx = np.random.default_rng(1).integers(0, g.M, size=200000)
@@ -327,3 +328,22 @@ def test_windowed_protocol_matches_oracle(sg, oracle_mod):
     assert rg.keys() == ro.keys() and len(rg) > 20
     for k in rg:
         assert rg[k][1] == ro[k][1] and np.array_equal(rg[k][0], ro[k][0]), k
+
+
+@pytest.mark.parametrize("log2n,W,T,sweeps", [(12, 16, 0.6, 256), (12, 16, 1.0, 256), (12, 16, 1.4, 256), (16, 16, 0.6, 8), (16, 16, 1.4, 8),
+                                              (20, 4, 1.4, 2)])
+def test_config5_sizes_and_temperatures(sg, oracle_mod, log2n, W, T, sweeps):
+    """BASELINE.json configs[4] (aging protocol sweep): the smaller sizes with their sample counts (Q17) at the
+    three temperatures, through the tw, t = 2^k schedule; seeds as in workloads.cfg5()."""
+    from paper_1906_11195_b200.workloads import cfg5, run_schedule
+
+    w = next(x for x in cfg5() if x.N == 1 << log2n and x.T == T)
+    assert w.n_words == W
+    g = sg.Sim(w.model, w.N, w.c, w.T, w.seed, w.n_words)
+    o = oracle_mod.Oracle(w.model, w.N, w.c, w.T, w.seed, w.n_words)
+    cg, co = run_schedule(g, sweeps), run_schedule(o, sweeps)
+    assert cg.keys() == co.keys()
+    for k in cg:
+        assert np.array_equal(cg[k], co[k]), k
+    _assert_same_state(g, o)
+    assert np.array_equal(g.energy(), o.energy())
