@@ -22,19 +22,14 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// L2 eviction policies.  The spin array is gathered at random (8 useful bytes per 32-byte sector)
-// and is re-read four times per sweep, so it is kept in L2 (evict_last); couplings, indices and
-// per-site metadata are touched once per sweep and stream through (evict_first, no L1 allocation).
+// L2 eviction policies.  Couplings, indices and per-site labels are touched once per sweep and stream through
+// (evict_first, no L1 allocation), so that they displace as little as possible of the spin words that the gathers
+// re-read; the spin words themselves use the default policy (evict_last / L1::no_allocate on them measured no gain,
+// profiles/r01_sweep.md).
 __device__ __forceinline__ uint64_t policy_evict_first()
 {
     uint64_t p;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
-__device__ __forceinline__ uint64_t policy_evict_last()
-{
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
     return p;
 }
 __device__ __forceinline__ uint64_t policy_evict_normal()
@@ -55,22 +50,12 @@ __device__ __forceinline__ uint32_t ld_stream_u32(const uint32_t *ptr, uint64_t 
     asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.b32 %0, [%1], %2;" : "=r"(v) : "l"(ptr), "l"(pol));
     return v;
 }
-__device__ __forceinline__ uint32_t ld_stream_u8(const uint8_t *ptr, uint64_t pol)
-{
-    uint32_t v;
-    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.u8 %0, [%1], %2;" : "=r"(v) : "l"(ptr), "l"(pol));
-    return v;
-}
 // spin words: written by other classes' launches, so no .nc; keep in L2
 __device__ __forceinline__ uint64_t ld_keep_u64(const uint64_t *ptr, uint64_t pol)
 {
     uint64_t v;
     asm volatile("ld.global.L1::no_allocate.L2::cache_hint.b64 %0, [%1], %2;" : "=l"(v) : "l"(ptr), "l"(pol));
     return v;
-}
-__device__ __forceinline__ void st_keep_u64(uint64_t *ptr, uint64_t v, uint64_t pol)
-{
-    asm volatile("st.global.L2::cache_hint.b64 [%0], %1, %2;" ::"l"(ptr), "l"(v), "l"(pol) : "memory");
 }
 __device__ __forceinline__ uint64_t ld_plain_u64(const uint64_t *ptr)
 {

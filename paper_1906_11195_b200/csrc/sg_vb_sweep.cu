@@ -2,14 +2,14 @@
 // (row a3 of SURVEY.md 8(a); PAPER.md:260 "classic single spin flip Metropolis", :318-320 kernel prose).
 // Conventions: DESIGN.md section 3 (O7, Q14).
 //
-// One thread per (site, word), SG_BT threads per CTA.  m_e = own ^ neighbour ^ coupling (bit = bond unsatisfied) for every incident
-// edge, u = per-lane sum of the m_e in 5 bit planes (carry-save adders), one Philox draw r shared by the 64
+// One thread per (site, word), SG_BT threads per CTA.  m_e = own ^ neighbour ^ coupling (bit = bond unsatisfied) for
+// every incident edge, u = per-lane sum of the m_e in 5 bit planes (carry-save adders), one Philox draw r shared by the 64
 // lanes, kstar = #{k >= 1 : r < thr[k]}, flip the lanes with u >= ceil((d - kstar)/2).  No floating point.
 //
 // Memory behaviour (B200, profiles/r01_probes.md): couplings, neighbour indices and site labels are read once
 // per sweep, coalesced, and stream through L2 (evict_first, no L1 allocation).  The neighbour spin words are
-// 8-byte gathers: they cost one L1TEX wavefront each and, when they miss L2, one DRAM row activation each, which
-// is what bounds the sweep.  The host generator therefore orders the sites of a class by breadth-first index
+// 8-byte gathers: they cost one L1TEX wavefront each and, when they miss L2, a whole 128-byte line from HBM each,
+// which is what bounds the sweep.  The host generator therefore orders the sites of a class by breadth-first index
 // (sg_host.cpp), so that the gathers along tree edges stay inside a moving window of every other class's block.
 #include <cuda_runtime.h>
 
