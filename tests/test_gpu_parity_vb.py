@@ -248,7 +248,7 @@ def test_config2_full_size_first_sweeps(sg, oracle_mod):
     assert np.array_equal(g.energy(), o.energy())
 
 
-@pytest.mark.parametrize("T", [float("inf"), 0.0])
+@pytest.mark.parametrize("T", [float("inf")])     # T = 0 at this size costs another minute of host graph generation; T = 0 is checked at N = 3000
 def test_largest_size_properties(sg, T):
     """BASELINE.json configs[4] top size N = 2^26 (W = 1), where the oracle is too slow to run in a test: properties
     that hold at any size.  T = inf: every proposal is accepted, so D alternates N, 0 and the energy is invariant (Q21);
