@@ -44,11 +44,11 @@ enum { SG_OK = 0, SG_EINVAL = -1, SG_ENOMEM = -2, SG_ECUDA = -3, SG_ESLOT = -4 }
  *                        bipartite graph of degree 4: halves {0..N/2-1} and {N/2..N-1},
  *                        four clash-free random permutations of one half onto the other (O2b), hence
  *                        exactly two colour classes; N even and >= 8; c is ignored.
- *   N       number of sites, 2 <= N < 2^31 (SK: N <= 32768 so that int16 local fields are exact).
+ *   N       number of sites, 2 <= N < 2^31 - 2 (SK: N <= 32768 so that int16 local fields are exact).
  *   c       mean degree (VB), c >= 0 and M <= N(N-1)/2.
  *   T       temperature, 0 <= T <= +inf (T = 0 and T = inf are legal).
  *   seed    Philox key.  (model, N, c, T, seed, n_words) determine every bit of every output.
- *   n_words 64-bit words per site, >= 1; lane l = 64*w + b is bit b of word w.
+ *   n_words 64-bit words per site, 1 <= n_words <= 65535; lane l = 64*w + b is bit b of word w.
  * Spins start uniformly random, sweep counter = 0.
  * Returns NULL on failure (bad argument, no CUDA device, out of memory).
  */
@@ -138,29 +138,38 @@ void sg_host_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t
 
 /*
  * The VB instance exactly as sg_create lays it out for the device, built on
- * the host only.  Sites are relabelled to positions p: class-major (colour 0, 1, ...), every class starting
- * at a multiple of 32, the gap positions being padding (orig = 0xFFFFFFFF).  Inside a class the sites keep
- * their breadth-first index order (BFS over the whole graph, roots in label order, rows in edge order): the
- * locality-improving relabelling; every window of `sort_window` consecutive sites of a class is then stably
- * sorted by degree.  Slice g = positions 32g .. 32g+31 has row length D = slice_ptr[g+1] - slice_ptr[g] = the
- * largest degree in the slice and stores its rows column-major: entry 32*slice_ptr[g] + 32*k + j is the k-th
- * neighbour (a position) of the j-th site of the slice.  Entries beyond a site's degree, and all entries of
- * padding positions, point at the site's own position with edge id 0xFFFFFFFF (coupling word 0).
- * No output depends on this relabelling: the Philox counter uses the original label (Q15).
+ * the host only.  Sites are relabelled to positions p = 0..N-1: class-major (colour 0, 1, ...), inside a class in
+ * breadth-first order (BFS over the whole graph, roots in label order, rows in edge order): the locality-improving
+ * relabelling.
+ * Gauge: the BFS forest's edges ("tree entries", T) carry no coupling word: with eps_root = 0 and
+ * eps_child = eps_parent ^ kappa_(tree edge) the device stores sigma ^ eps and kappa_ij ^ eps_i ^ eps_j, which leaves
+ * every bond state sigma_i ^ sigma_j ^ kappa_ij, hence every output, unchanged.  The other entries ("X") keep a word.
+ * Slices: every class is cut greedily, in position order, into runs of at most 32 sites whose T entries and whose X
+ * entries number at most `cap` each (cap depends on n_words only).  hdr[g] = 4 uint32: first position, first index in
+ * col, first coupling entry, and n | nTs << 6 | nXs << 16 (sites, T entries, X entries of the slice); one sentinel
+ * follows the last slice.  col holds, slice after slice, the T entries in site order (per site: parent first, then the
+ * children by ascending position), then the X entries in site order (per site by ascending position); the coupling
+ * entries follow the X order, jeid gives the edge id of each.  orig_s[32g + j] = label of the j-th site of slice g
+ * (0xFFFFFFFF for j >= n); rp_s[32g + j] = tOff | xOff << 10 | nT << 20 | nX << 25: where the site's entries start
+ * inside the slice's T run / X run, and how many there are.  No output depends on any of this: the Philox counter
+ * uses the original label (Q15).
  */
 typedef struct sg_host_graph sg_host_graph;
-sg_host_graph *sg_host_graph_create(int model, uint64_t N, double c, uint64_t seed);   /* model: SG_MODEL_VB or SG_MODEL_RRBG; NULL on bad arguments */
+/* model: SG_MODEL_VB or SG_MODEL_RRBG; NULL on bad arguments */
+sg_host_graph *sg_host_graph_create(int model, uint64_t N, double c, uint64_t seed, uint32_t n_words);
 void sg_host_graph_destroy(sg_host_graph *g);
-/* info HOST 8 uint64: M, K (colours), dmax, entries, nslices, N, P (positions incl. padding), sort_window */
+/* info HOST 9 uint64: M, K (colours), dmax, entries (length of col = 2M), nslices, N, nJ (coupling entries), cap, gauge (1/0) */
 int sg_host_graph_info(const sg_host_graph *g, uint64_t *info);
 /*
- * Copies out whichever arrays are non-NULL (all HOST): u,v M uint32; colour N uint32; orig P uint32
- * (position -> label); deg P uint32 (per position, 0 for padding); slice_ptr nslices+1 uint32; col entries
- * uint32; eid entries uint32; class_pos0, class_n, class_slice0 K uint64 each.
+ * Copies out whichever arrays are non-NULL (all HOST): u,v M uint32; colour N uint32; orig N uint32
+ * (position -> label); hdr 4*(nslices+1) uint32; orig_s, rp_s 32*nslices uint32; col entries uint32; jeid nJ uint32;
+ * tpar, teid N uint32 (parent position / tree edge id, 0xFFFFFFFF for roots); bfs_pos N uint32 (positions in
+ * breadth-first order); class_pos0, class_n, class_slice0, class_nslices K uint64 each.
  */
 int sg_host_graph_get(const sg_host_graph *g, uint32_t *u, uint32_t *v, uint32_t *colour, uint32_t *orig,
-                      uint32_t *deg, uint32_t *slice_ptr, uint32_t *col, uint32_t *eid,
-                      uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0);
+                      uint32_t *hdr, uint32_t *orig_s, uint32_t *rp_s, uint32_t *col, uint32_t *jeid,
+                      uint32_t *tpar, uint32_t *teid, uint32_t *bfs_pos,
+                      uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0, uint64_t *class_nslices);
 
 /*
  * Number of kernels this library has launched (process-wide, all handles) since load.

@@ -14,7 +14,7 @@ SG_OK, SG_EINVAL, SG_ENOMEM, SG_ECUDA, SG_ESLOT = 0, -1, -2, -3, -4
 SG_MAX_SLOTS = 64
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libsg.so")
+LIB_PATH = os.environ.get("SG_LIBSG_PATH") or os.path.join(_HERE, "libsg.so")   # the override serves A/B measurements of builds
 
 # every symbol include/sg.h declares: (name, restype, argtypes)
 _u64, _u32, _i32, _dbl, _vp = C.c_uint64, C.c_uint32, C.c_int32, C.c_double, C.c_void_p
@@ -39,10 +39,10 @@ SYMBOLS = {
     "sg_get_thresholds": (C.c_int, [_vp, _vp, _u64]),
     "sg_kernel_launches": (_u64, []),
     "sg_host_philox": (None, [_u32] * 6 + [_vp]),
-    "sg_host_graph_create": (_vp, [C.c_int, _u64, _dbl, _u64]),
+    "sg_host_graph_create": (_vp, [C.c_int, _u64, _dbl, _u64, _u32]),
     "sg_host_graph_destroy": (None, [_vp]),
     "sg_host_graph_info": (C.c_int, [_vp, _vp]),
-    "sg_host_graph_get": (C.c_int, [_vp] * 12),
+    "sg_host_graph_get": (C.c_int, [_vp] * 17),
 }
 
 
@@ -229,28 +229,27 @@ def host_philox(c0, c1, c2, c3, k0, k1) -> np.ndarray:
     return out
 
 
-def host_graph(N: int, c: float, seed: int, model: int = SG_MODEL_VB) -> dict:
-    """The device layout of a VB instance, built by the library's host generator only."""
+def host_graph(N: int, c: float, seed: int, model: int = SG_MODEL_VB, n_words: int = 1) -> dict:
+    """The device layout of a VB instance (include/sg.h, sg_host_graph_*), built by the library's host generator only."""
     L = load_library()
-    g = L.sg_host_graph_create(int(model), int(N), float(c), int(seed))
+    g = L.sg_host_graph_create(int(model), int(N), float(c), int(seed), int(n_words))
     if not g:
         raise SGError(SG_EINVAL, _err())
     try:
-        info = np.zeros(8, dtype=np.uint64)
+        info = np.zeros(9, dtype=np.uint64)
         _check(L.sg_host_graph_info(g, _ptr(info)))
-        M, K, dmax, entries, nslices, N, P, sort_window = (int(x) for x in info)
-        a = dict(M=M, K=K, dmax=dmax, entries=entries, nslices=nslices, N=N, P=P, sort_window=sort_window)
+        M, K, dmax, entries, nslices, N, nJ, cap, gauge = (int(x) for x in info)
+        a = dict(M=M, K=K, dmax=dmax, entries=entries, nslices=nslices, N=N, nJ=nJ, cap=cap, gauge=gauge)
         a["u"] = np.zeros(M, np.uint32); a["v"] = np.zeros(M, np.uint32)
-        a["colour"] = np.zeros(N, np.uint32)
-        for k in ("orig", "deg"):
-            a[k] = np.zeros(P, np.uint32)
-        a["slice_ptr"] = np.zeros(nslices + 1, np.uint32)
-        a["col"] = np.zeros(entries, np.uint32); a["eid"] = np.zeros(entries, np.uint32)
-        for k in ("class_pos0", "class_n", "class_slice0"):
+        for k in ("colour", "orig", "tpar", "teid", "bfs_pos"):
+            a[k] = np.zeros(N, np.uint32)
+        a["hdr"] = np.zeros((nslices + 1, 4), np.uint32)
+        a["orig_s"] = np.zeros(32 * nslices, np.uint32); a["rp_s"] = np.zeros(32 * nslices, np.uint32)
+        a["col"] = np.zeros(entries, np.uint32); a["jeid"] = np.zeros(nJ, np.uint32)
+        for k in ("class_pos0", "class_n", "class_slice0", "class_nslices"):
             a[k] = np.zeros(K, np.uint64)
-        _check(L.sg_host_graph_get(g, _ptr(a["u"]), _ptr(a["v"]), _ptr(a["colour"]), _ptr(a["orig"]), _ptr(a["deg"]),
-                                   _ptr(a["slice_ptr"]), _ptr(a["col"]), _ptr(a["eid"]), _ptr(a["class_pos0"]),
-                                   _ptr(a["class_n"]), _ptr(a["class_slice0"])))
+        _check(L.sg_host_graph_get(g, *(_ptr(a[k]) for k in ("u", "v", "colour", "orig", "hdr", "orig_s", "rp_s", "col", "jeid", "tpar",
+                                                              "teid", "bfs_pos", "class_pos0", "class_n", "class_slice0", "class_nslices"))))
         return a
     finally:
         L.sg_host_graph_destroy(g)

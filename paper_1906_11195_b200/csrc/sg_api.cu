@@ -30,42 +30,62 @@ void destroy_impl(sg_sim *h)
     delete h;
 }
 
+// kappa_e[w] of DESIGN.md O3 on the host (the gauge needs the tree edges' couplings before anything is on the device)
+uint64_t host_coupling_word(uint32_t e, uint32_t w, SGSeed key)
+{
+    const Philox4 x = sg_philox_host(e, w, 0u, 2u << 24, key.k0, key.k1);
+    return (uint64_t)x.x[0] | ((uint64_t)x.x[1] << 32);
+}
+
 int create_vb(sg_sim *h)
 {
     cudaStream_t st = sgx_stream();
-    if (!sg_build_vb_graph(h->graph_model, h->N, h->c, h->seed, h->g)) return SG_EINVAL;
+    if (!sg_build_vb_graph(h->graph_model, h->N, h->c, h->seed, h->W, h->g)) return SG_EINVAL;
     VBHostGraph &g = h->g;
     h->M = g.M;
-    const uint64_t W = h->W, P = g.P;
-    const uint64_t entries = g.col.size();
-    const uint64_t nslices = g.slice_ptr.size() - 1;
-    h->spin_words = P * W;
-    h->vb_entries = entries;
-    h->vb.spin = dev_alloc<uint64_t>(h, P * W);
-    h->vb.J = dev_alloc<uint64_t>(h, entries * W + 1);
+    const uint64_t W = h->W, N = g.N;
+    const uint64_t nslices = g.hdr.size() - 1, entries = g.col.size(), nJ = g.jeid.size();
+    h->spin_words = N * W;
+    h->vb_nJ = nJ;
+    h->vb.nslices = (uint32_t)nslices;
+    h->vb.cap = g.cap;
+    h->vb.spin = dev_alloc<uint64_t>(h, N * W);
+    h->vb.eps = dev_alloc<uint64_t>(h, N * W);
+    h->vb.J = dev_alloc<uint64_t>(h, nJ * W + 4);
     h->vb.col = dev_alloc<uint32_t>(h, entries + 1);
-    h->vb.orig = dev_alloc<uint32_t>(h, P);
-    h->vb.slice_ptr = dev_alloc<uint32_t>(h, nslices + 1);
-    h->vb.thr = dev_alloc<uint64_t>(h, 33);
-    uint32_t *eid_dev = dev_alloc<uint32_t>(h, entries + 1);
-    if (!h->vb.spin || !h->vb.J || !h->vb.col || !h->vb.orig || !h->vb.slice_ptr || !h->vb.thr || !eid_dev)
+    h->vb.orig = dev_alloc<uint32_t>(h, N);
+    h->vb.orig_s = dev_alloc<uint32_t>(h, 32 * nslices);
+    h->vb.rp_s = dev_alloc<uint32_t>(h, 32 * nslices);
+    h->vb.hdr = dev_alloc<SGHdr>(h, nslices + 1);
+    uint32_t *jeid_dev = dev_alloc<uint32_t>(h, nJ + 1);
+    if (!h->vb.spin || !h->vb.eps || !h->vb.J || !h->vb.col || !h->vb.orig || !h->vb.orig_s || !h->vb.rp_s || !h->vb.hdr || !jeid_dev)
         return SG_ENOMEM;
     h->thr_host = sg_vb_thresholds(h->T, g.dmax);
-    std::vector<uint64_t> thr33(33, 0);
-    for (size_t k = 0; k < h->thr_host.size() && k < 33; ++k) thr33[k] = h->thr_host[k];
-    if (!upload(h->vb.col, g.col, st) || !upload(h->vb.orig, g.orig, st) ||
-        !upload(h->vb.slice_ptr, g.slice_ptr, st) || !upload(h->vb.thr, thr33, st) || !upload(eid_dev, g.eid, st))
+    for (size_t k = 0; k < h->thr_host.size() && k < 32; ++k) h->vb.thr_host[k] = h->thr_host[k];
+    // the gauge: eps_root = 0, eps_child = eps_parent ^ kappa_(tree edge), parents before children (sg_internal.h)
+    std::vector<uint64_t> eps(N * W, 0);
+    if (g.gauge)
+        for (uint64_t q = 0; q < N; ++q) {
+            const uint64_t p = g.bfs_pos[q], par = g.tpar[p];
+            if (par == SG_NONE) continue;
+            for (uint32_t w = 0; w < W; ++w) eps[p * W + w] = eps[par * W + w] ^ host_coupling_word(g.teid[p], w, h->key);
+        }
+    if (!upload(h->vb.col, g.col, st) || !upload(h->vb.orig, g.orig, st) || !upload(h->vb.orig_s, g.orig_s, st) ||
+        !upload(h->vb.rp_s, g.rp_s, st) || !upload(h->vb.hdr, g.hdr, st) ||
+        !upload(jeid_dev, g.jeid, st) || !upload(h->vb.eps, eps, st))
         return SG_ECUDA;
-    int rc = sgk_init_vb_couplings(h->vb.J, eid_dev, entries, h->W, h->key, st);
+    int rc = sgk_init_vb_couplings(h->vb, jeid_dev, h->W, h->key, st);
     if (rc) return rc;
-    rc = sgk_init_spins(h->vb.spin, h->vb.orig, P, h->W, h->key, st);
+    rc = sgk_init_spins(h->vb.spin, h->vb.orig, h->vb.eps, N, h->W, h->key, st);
     if (rc) return rc;
     if (!cuda_ok(cudaStreamSynchronize(st), "sg_create")) return SG_ECUDA;
-    // the entry->edge table is only needed to draw the couplings; col/eid host copies are large: drop them
-    sgx_free(eid_dev);
-    h->owned.erase(std::find(h->owned.begin(), h->owned.end(), (void *)eid_dev));
-    std::vector<uint32_t>().swap(g.eid);
+    // the entry->edge table is only needed to draw the couplings; the large host copies are not needed any more
+    sgx_free(jeid_dev);
+    h->owned.erase(std::find(h->owned.begin(), h->owned.end(), (void *)jeid_dev));
+    std::vector<uint32_t>().swap(g.jeid);
     std::vector<uint32_t>().swap(g.col);
+    std::vector<uint32_t>().swap(g.bfs_pos);
+    std::vector<uint32_t>().swap(g.orig_s);
     return SG_OK;
 }
 
@@ -75,8 +95,8 @@ extern "C" sg_sim *sg_create(int model, uint64_t N, double c, double T, uint64_t
 {
     g_err.clear();
     if (model != SG_MODEL_VB && model != SG_MODEL_SK && model != SG_MODEL_RRBG) { sg_set_error("sg_create: unknown model"); return nullptr; }
-    if (N < 2 || N >= (1ull << 31)) { sg_set_error("sg_create: N must satisfy 2 <= N < 2^31"); return nullptr; }
-    if (n_words == 0) { sg_set_error("sg_create: n_words must be >= 1"); return nullptr; }
+    if (N < 2 || N >= (1ull << 31) - 2) { sg_set_error("sg_create: N must satisfy 2 <= N < 2^31 - 2"); return nullptr; }
+    if (n_words == 0 || n_words > 65535) { sg_set_error("sg_create: n_words must satisfy 1 <= n_words <= 65535"); return nullptr; }
     if (!(T >= 0.0)) { sg_set_error("sg_create: T must be >= 0 (T = inf allowed)"); return nullptr; }
     if (model == SG_MODEL_SK && N > 32768) { sg_set_error("sg_create: SK needs N <= 32768 (int16 local fields)"); return nullptr; }
     std::string why;
@@ -113,7 +133,7 @@ extern "C" int sg_sweep(sg_sim *h, uint64_t n)
     cudaStream_t st = sgx_stream();
     for (uint64_t it = 0; it < n; ++it) {
         for (uint32_t k = 0; k < h->g.K; ++k) {
-            const int rc = sgk_vb_sweep_class(h->vb, h->g.cls[k], h->g.P, h->vb_entries, h->W, h->sweep, h->key, h->vb_reverse, st);
+            const int rc = sgk_vb_sweep_class(h->vb, h->g.cls[k], h->g.N, h->vb_nJ, h->W, h->sweep, h->key, h->vb_reverse, st);
             h->vb_reverse = !h->vb_reverse;
             if (rc) return rc;
         }
@@ -148,7 +168,7 @@ extern "C" int sg_correlation(sg_sim *h, uint32_t slot, uint64_t *out_counts)
     if (!cuda_ok(cudaMemsetAsync(h->counts_dev, 0, lanes * 8, st), "sg_correlation")) return SG_ECUDA;
     if (h->model == SG_MODEL_SK) return sg_sk_correlation_impl(h, h->slot[slot], out_counts);
     // position order in both operands (the same permutation), so no relabelling is needed
-    const int rc = sgk_xor_popcount(current_config(h), h->slot[slot], h->g.P, h->W, h->counts_dev, st);
+    const int rc = sgk_xor_popcount(current_config(h), h->slot[slot], h->g.N, h->W, h->counts_dev, st);
     if (rc) return rc;
     if (!cuda_ok(cudaMemcpyAsync(out_counts, h->counts_dev, lanes * 8, cudaMemcpyDeviceToHost, st), "sg_correlation") ||
         !cuda_ok(cudaStreamSynchronize(st), "sg_correlation"))
@@ -163,10 +183,8 @@ extern "C" int sg_energy(sg_sim *h, int64_t *out)
     cudaStream_t st = sgx_stream();
     const uint64_t lanes = 64ull * h->W;
     if (!cuda_ok(cudaMemsetAsync(h->counts_dev, 0, lanes * 8, st), "sg_energy")) return SG_ECUDA;
-    for (uint32_t k = 0; k < h->g.K; ++k) {
-        const int rc = sgk_vb_unsat_class(h->vb, h->g.cls[k], h->W, h->counts_dev, st);
-        if (rc) return rc;
-    }
+    const int rc = sgk_vb_unsat(h->vb, h->g.N, h->vb_nJ, h->W, h->counts_dev, st);
+    if (rc) return rc;
     std::vector<uint64_t> twoU(lanes);
     if (!cuda_ok(cudaMemcpyAsync(twoU.data(), h->counts_dev, lanes * 8, cudaMemcpyDeviceToHost, st), "sg_energy") ||
         !cuda_ok(cudaStreamSynchronize(st), "sg_energy"))
@@ -204,7 +222,7 @@ extern "C" int sg_get_spins(sg_sim *h, int32_t slot, uint64_t *out)
     cudaStream_t st = sgx_stream();
     if (h->model == SG_MODEL_SK) return sg_sk_get_spins_impl(h, src, out);
     if (!ensure_scratch(h)) return SG_ENOMEM;
-    const int rc = sgk_permute_words(src, h->scratch, h->vb.orig, h->g.P, h->W, /*scatter=*/true, st);
+    const int rc = sgk_permute_words(src, h->scratch, h->vb.orig, h->vb.eps, h->g.N, h->W, /*scatter=*/true, st);
     if (rc) return rc;
     if (!cuda_ok(cudaMemcpyAsync(out, h->scratch, h->N * h->W * 8, cudaMemcpyDeviceToHost, st), "sg_get_spins") ||
         !cuda_ok(cudaStreamSynchronize(st), "sg_get_spins"))
@@ -219,7 +237,7 @@ extern "C" int sg_set_spins(sg_sim *h, const uint64_t *in)
     cudaStream_t st = sgx_stream();
     if (!ensure_scratch(h)) return SG_ENOMEM;
     if (!cuda_ok(cudaMemcpyAsync(h->scratch, in, h->N * h->W * 8, cudaMemcpyHostToDevice, st), "sg_set_spins")) return SG_ECUDA;
-    const int rc = sgk_permute_words(h->scratch, h->vb.spin, h->vb.orig, h->g.P, h->W, /*scatter=*/false, st);
+    const int rc = sgk_permute_words(h->scratch, h->vb.spin, h->vb.orig, h->vb.eps, h->g.N, h->W, /*scatter=*/false, st);
     if (rc) return rc;
     if (!cuda_ok(cudaStreamSynchronize(st), "sg_set_spins")) return SG_ECUDA;
     return SG_OK;
@@ -254,18 +272,53 @@ extern "C" int sg_get_couplings(sg_sim *h, uint64_t *out)
 {
     if (!h || !out) { sg_set_error("sg_get_couplings: null argument"); return SG_EINVAL; }
     if (h->model == SG_MODEL_SK) return sg_sk_get_couplings_impl(h, out);
+    // Undo the gauge from what the device holds: a coupling entry of the site at position p towards position nb stores
+    // kappa ^ eps[p] ^ eps[nb]; a tree edge stores nothing and has kappa = eps[p] ^ eps[parent].  Every edge that is
+    // not a tree edge is stored at both endpoints; the two copies must agree.
     cudaStream_t st = sgx_stream();
-    const uint64_t entries = 32ull * h->g.slice_ptr.back();
-    std::vector<uint64_t> J(entries * h->W);
+    const VBHostGraph &g = h->g;
+    const uint64_t W = h->W, N = g.N, nslices = g.hdr.size() - 1, entries = g.hdr[nslices].col_off, nJ = g.hdr[nslices].j_off;
+    std::vector<uint64_t> J(nJ * W), eps(N * W);
+    std::vector<uint32_t> col(entries);
     if (!cuda_ok(cudaMemcpyAsync(J.data(), h->vb.J, J.size() * 8, cudaMemcpyDeviceToHost, st), "sg_get_couplings") ||
+        !cuda_ok(cudaMemcpyAsync(eps.data(), h->vb.eps, eps.size() * 8, cudaMemcpyDeviceToHost, st), "sg_get_couplings") ||
+        !cuda_ok(cudaMemcpyAsync(col.data(), h->vb.col, col.size() * 4, cudaMemcpyDeviceToHost, st), "sg_get_couplings") ||
         !cuda_ok(cudaStreamSynchronize(st), "sg_get_couplings"))
         return SG_ECUDA;
-    const uint32_t W = h->W;
-    for (uint64_t e = 0; e < h->g.M; ++e) {
-        const uint64_t ent = h->g.entry_of_edge[e];
-        const uint64_t col32 = ent / 32, j = ent % 32;
-        for (uint32_t w = 0; w < W; ++w) out[e * W + w] = J[(col32 * 32) * W + j * W + w];
+    std::vector<uint8_t> seen(g.M, 0);
+    auto edge_between = [&](uint32_t i, uint32_t v) -> uint32_t {
+        for (uint64_t a = g.row_ptr[i]; a < g.row_ptr[i + 1]; ++a)
+            if (g.adj[a] == v) return g.adj_e[a];
+        return SG_NONE;
+    };
+    for (uint64_t s = 0; s < nslices; ++s) {
+        const SGHdr &hd = g.hdr[s];
+        const uint32_t n = hd.counts & 63u, nTs = (hd.counts >> 6) & 1023u;
+        for (uint32_t j = 0; j < n; ++j) {
+            const uint32_t rp = g.rp_s[32 * s + j], xOff = (rp >> 10) & 1023u, nX = rp >> 25;
+            const uint64_t p = (uint64_t)hd.pos0 + j;
+            for (uint32_t r = 0; r < nX; ++r) {
+                const uint64_t nb = col[(uint64_t)hd.col_off + nTs + xOff + r], x = (uint64_t)hd.j_off + xOff + r;
+                const uint32_t e = edge_between(g.orig[p], g.orig[nb]);
+                if (e == SG_NONE) { sg_set_error("sg_get_couplings: a stored entry is not an edge of the graph"); return SG_ECUDA; }
+                for (uint32_t w = 0; w < W; ++w) {
+                    const uint64_t k = J[x * W + w] ^ eps[p * W + w] ^ eps[nb * W + w];
+                    if (seen[e] && out[(uint64_t)e * W + w] != k) { sg_set_error("sg_get_couplings: the two stored copies of an edge differ"); return SG_ECUDA; }
+                    out[(uint64_t)e * W + w] = k;
+                }
+                seen[e]++;
+            }
+        }
     }
+    for (uint64_t p = 0; p < N; ++p) {
+        if (!g.gauge || g.tpar[p] == SG_NONE) continue;
+        const uint32_t e = g.teid[p];
+        if (seen[e]) { sg_set_error("sg_get_couplings: a tree edge also has a stored coupling"); return SG_ECUDA; }
+        for (uint32_t w = 0; w < W; ++w) out[(uint64_t)e * W + w] = eps[p * W + w] ^ eps[(uint64_t)g.tpar[p] * W + w];
+        seen[e] = 2;
+    }
+    for (uint64_t e = 0; e < g.M; ++e)
+        if (seen[e] != 2) { sg_set_error("sg_get_couplings: an edge is not stored exactly twice"); return SG_ECUDA; }
     return SG_OK;
 }
 

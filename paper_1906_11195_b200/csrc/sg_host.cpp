@@ -81,11 +81,24 @@ struct PairSet {
 };
 }  // namespace
 
-// O2b: random regular bipartite graph of degree 4 as the union of four permutations of
-// half A = {0..H-1} onto half B = {H..N-1}, H = N/2, without a repeated pair.  Permutation a = 0..3: attempts
-// t = 0,1,2,... (one counter over all four); an attempt is a Fisher-Yates shuffle of the identity, for i = H-1 down
-// to 1: j = (x*(i+1)) >> 32 with x = word n&3 of P(n>>2, t, 0, tag 4), n = H-1-i, swap(perm[i], perm[j]); it is
-// accepted if it differs from every earlier accepted permutation at every i.  Edge e = a*H + i joins i and H + perm_a[i].
+// O2b: random regular bipartite graph of degree 4: four perfect matchings between half
+// A = {0..H-1} and half B = {H..N-1}, H = N/2, no pair matched twice.  DESIGN.md O2b fixes the draw: candidate number t
+// (t = 0, 1, 2, ... over all four matchings) is the identity run through the swap sequence
+//   position H-1-n  <->  position (x_n * (H-n)) >> 32,   n = 0 .. H-2,   x_n = word n&3 of P(n>>2, t, 0, tag 4),
+// and a candidate is kept if no A-vertex gets a partner it already has.  Edge e = a*H + i joins i and H + m_a(i).
+namespace {
+// the swap targets of candidate t, one Philox block per four consecutive swaps
+void rrbg_swap_targets(uint64_t H, uint64_t t, uint32_t k0, uint32_t k1, std::vector<uint32_t> &target)
+{
+    target.resize(H > 0 ? H - 1 : 0);
+    for (uint64_t n0 = 0; n0 + 1 < H; n0 += 4) {
+        const Philox4 blk = sg_philox_host((uint32_t)(n0 >> 2), (uint32_t)t, 0u, 4u << 24, k0, k1);
+        for (uint64_t n = n0; n < std::min<uint64_t>(n0 + 4, H - 1); ++n)
+            target[n] = (uint32_t)(((uint64_t)blk.x[n - n0] * (H - n)) >> 32);
+    }
+}
+}  // namespace
+
 static bool build_rrbg_edges(uint64_t N, uint64_t seed, VBHostGraph &g)
 {
     if (N < 8 || (N & 1)) { sg_set_error("sg_create: the RRBG model needs an even N >= 8"); return false; }
@@ -93,28 +106,24 @@ static bool build_rrbg_edges(uint64_t N, uint64_t seed, VBHostGraph &g)
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     g.N = N; g.M = 4 * H;
     g.eu.resize(g.M); g.ev.resize(g.M);
-    std::vector<uint32_t> perm(H);
-    uint64_t t = 0;
-    for (uint32_t a = 0; a < 4; ++a) {
-        for (;; ++t) {
-            std::iota(perm.begin(), perm.end(), 0u);
-            Philox4 x{{0, 0, 0, 0}};
-            for (uint64_t i = H - 1; i >= 1; --i) {
-                const uint64_t n = H - 1 - i;
-                if ((n & 3) == 0) x = sg_philox_host((uint32_t)(n >> 2), (uint32_t)t, 0u, 4u << 24, k0, k1);
-                const uint64_t j = ((uint64_t)x.x[n & 3] * (i + 1)) >> 32;
-                std::swap(perm[i], perm[j]);
-            }
-            bool clash = false;
-            for (uint32_t b = 0; b < a && !clash; ++b)
-                for (uint64_t i = 0; i < H; ++i)
-                    if (g.ev[(uint64_t)b * H + i] == (uint32_t)(H + perm[i])) { clash = true; break; }
-            if (!clash) { ++t; break; }
-        }
+    std::vector<uint32_t> partner(4 * H);          // partner[4 i + a] = B-index matched to A-vertex i by matching a
+    std::vector<uint32_t> cand(H), target;
+    uint32_t kept = 0;
+    for (uint64_t t = 0; kept < 4; ++t) {
+        rrbg_swap_targets(H, t, k0, k1, target);
+        for (uint64_t i = 0; i < H; ++i) cand[i] = (uint32_t)i;
+        for (uint64_t n = 0; n + 1 < H; ++n) std::swap(cand[H - 1 - n], cand[target[n]]);
+        bool fresh = true;
+        for (uint64_t i = 0; i < H && fresh; ++i)
+            for (uint32_t a = 0; a < kept; ++a)
+                if (partner[4 * i + a] == cand[i]) { fresh = false; break; }
+        if (!fresh) continue;
         for (uint64_t i = 0; i < H; ++i) {
-            g.eu[(uint64_t)a * H + i] = (uint32_t)i;
-            g.ev[(uint64_t)a * H + i] = (uint32_t)(H + perm[i]);
+            partner[4 * i + kept] = cand[i];
+            g.eu[(uint64_t)kept * H + i] = (uint32_t)i;
+            g.ev[(uint64_t)kept * H + i] = (uint32_t)(H + cand[i]);
         }
+        ++kept;
     }
     return true;
 }
@@ -145,7 +154,7 @@ static bool build_er_edges(uint64_t N, double c, uint64_t seed, VBHostGraph &g)
     return true;
 }
 
-bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, VBHostGraph &g)
+bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t n_words, VBHostGraph &g)
 {
     if (model == SG_MODEL_RRBG ? !build_rrbg_edges(N, seed, g) : !build_er_edges(N, c, seed, g)) return false;
     const uint64_t M = g.M;
@@ -180,15 +189,13 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, VBHostGra
     // Locality order (the "locality-improving relabelling within each colour class" of BASELINE.json): breadth-first
     // index over the whole graph, roots in label order, rows in stored order.  The graph is locally tree-like, so
     // a site's tree parent and children get nearby indices; since a class keeps this order, the gathers along the
-    // N-1 tree edges (half of all gathers at c = 4) walk through every other class's block monotonically and find
-    // their 32-byte sectors still in L2 (or L1) instead of costing a DRAM row activation each.
-    // (SG_VB_ORDER=label keeps the label order instead: a measurement knob, see profiles/; outputs are identical.)
+    // N-1 tree edges (half of all gathers at c = 4) walk through every other class's block monotonically: the
+    // lanes of a warp share 128-byte lines and the lines are still in L1/L2 when the next slices need them.
+    // The same forest fixes the gauge (see sg_internal.h): its edges need no coupling word.
+    // (SG_VB_ORDER=label keeps the label order for the positions: a measurement knob; outputs are identical.)
     std::vector<uint32_t> bfs; bfs.reserve(N);
-    const char *order_env = std::getenv("SG_VB_ORDER");
-    if (order_env && !std::strcmp(order_env, "label")) {
-        bfs.resize(N);
-        std::iota(bfs.begin(), bfs.end(), 0u);
-    } else {
+    std::vector<uint32_t> par(N, SG_NONE), par_e(N, SG_NONE);
+    {
         std::vector<uint8_t> seen(N, 0);
         for (uint64_t r = 0; r < N; ++r) {
             if (seen[r]) continue;
@@ -199,96 +206,100 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, VBHostGra
                 const uint32_t u = bfs[head++];
                 for (uint64_t a = g.row_ptr[u]; a < g.row_ptr[u + 1]; ++a) {
                     const uint32_t v = g.adj[a];
-                    if (!seen[v]) { seen[v] = 1; bfs.push_back(v); }
+                    if (!seen[v]) { seen[v] = 1; par[v] = u; par_e[v] = g.adj_e[a]; bfs.push_back(v); }
                 }
             }
         }
     }
-    // Positions: class-major; inside a class the sites keep the BFS order, except that every window of
-    // SG_SORT_WINDOW consecutive sites is stably sorted by degree, so that the 32 sites of a slice have (almost
-    // always) one degree and the sliced-ELL rows carry ~1 % padding.  Classes start at multiples of 32; the gap
-    // positions are padding (orig = NONE, spin word 0, never written).
+    const char *order_env = std::getenv("SG_VB_ORDER");
+    const bool label_order = order_env && !std::strcmp(order_env, "label");
+    const char *gauge_env = std::getenv("SG_VB_GAUGE");
+    g.gauge = !(gauge_env && !std::strcmp(gauge_env, "0"));                 // measurement knob: keep every coupling word
+    const char *cap_env = std::getenv("SG_VB_CAP");                          // measurement knob: entry budget of a slice
+    g.cap = cap_env ? (uint32_t)std::min(1023, std::max(31, std::atoi(cap_env))) : sg_vb_slice_cap(n_words);
+
+    // per site: tree entries nT (parent + children); the others are X entries
+    std::vector<uint8_t> nT(N, 0);
+    if (g.gauge)
+        for (uint64_t i = 0; i < N; ++i)
+            if (par[i] != SG_NONE) { nT[i]++; nT[par[i]]++; }
+    // positions: (class, breadth-first index)
     std::vector<uint64_t> ccount(K, 0);
     for (uint64_t i = 0; i < N; ++i) ccount[g.colour[i]]++;
     g.cls.assign(K, VBClass{});
-    uint64_t P = 0;
-    for (uint32_t k = 0; k < K; ++k) {
-        g.cls[k].pos0 = P;
-        g.cls[k].n = (ccount[k] + 31) / 32 * 32;
-        P += g.cls[k].n;
+    {
+        uint64_t p0 = 0;
+        for (uint32_t k = 0; k < K; ++k) { g.cls[k].pos0 = p0; g.cls[k].n = ccount[k]; p0 += ccount[k]; }
     }
-    if (P >= (1ull << 31)) { sg_set_error("sg_create: too many sites"); return false; }
-    g.P = P;
-    g.orig.assign(P, SG_NONE); g.pos.resize(N); g.deg.assign(P, 0);
+    g.orig.resize(N); g.pos.resize(N);
     {
         std::vector<uint64_t> fill(K);
         for (uint32_t k = 0; k < K; ++k) fill[k] = g.cls[k].pos0;
-        for (uint64_t q = 0; q < N; ++q) g.orig[fill[g.colour[bfs[q]]]++] = bfs[q];
-        const uint64_t SW = SG_SORT_WINDOW;
-        std::vector<uint32_t> tmp(SW);
-        for (uint32_t k = 0; k < K; ++k) {
-            const uint64_t p0 = g.cls[k].pos0, p1 = p0 + ccount[k];
-            for (uint64_t w0 = p0; w0 < p1; w0 += SW) {
-                const uint64_t w1 = std::min<uint64_t>(p1, w0 + SW);
-                uint32_t hist[33] = {0};
-                for (uint64_t p = w0; p < w1; ++p) hist[g.row_ptr[g.orig[p] + 1] - g.row_ptr[g.orig[p]] + 1]++;
-                for (int d = 0; d < 32; ++d) hist[d + 1] += hist[d];
-                for (uint64_t p = w0; p < w1; ++p) tmp[hist[g.row_ptr[g.orig[p] + 1] - g.row_ptr[g.orig[p]]]++] = g.orig[p];
-                std::copy(tmp.begin(), tmp.begin() + (w1 - w0), g.orig.begin() + w0);
-            }
-        }
-        for (uint64_t p = 0; p < P; ++p)
-            if (g.orig[p] != SG_NONE) {
-                g.pos[g.orig[p]] = (uint32_t)p;
-                g.deg[p] = (uint8_t)(g.row_ptr[g.orig[p] + 1] - g.row_ptr[g.orig[p]]);
-            }
+        if (label_order) for (uint64_t i = 0; i < N; ++i) g.orig[fill[g.colour[i]]++] = (uint32_t)i;
+        else for (uint64_t q = 0; q < N; ++q) g.orig[fill[g.colour[bfs[q]]]++] = bfs[q];
+        for (uint64_t p = 0; p < N; ++p) g.pos[g.orig[p]] = (uint32_t)p;
     }
+    g.tpar.assign(N, SG_NONE); g.teid.assign(N, SG_NONE);
+    g.bfs_pos.resize(N);
+    for (uint64_t q = 0; q < N; ++q) g.bfs_pos[q] = g.pos[bfs[q]];
     std::vector<uint32_t>().swap(bfs);
-    // sliced ELL: slice s = positions 32 s .. 32 s + 31, row length = the largest degree in the slice
-    const uint64_t nslices = P / 32;
-    g.slice_ptr.assign(nslices + 1, 0);
-    for (uint64_t s = 0; s < nslices; ++s) {
-        uint32_t D = 0;
-        for (uint32_t j = 0; j < 32; ++j) D = std::max<uint32_t>(D, g.deg[32 * s + j]);
-        const uint64_t next = (uint64_t)g.slice_ptr[s] + D;
-        if (next > 0x7FFFFFFull) { sg_set_error("sg_create: instance too large for 32-bit entry indices"); return false; }
-        g.slice_ptr[s + 1] = (uint32_t)next;
+    for (uint64_t p = 0; p < N; ++p) {
+        const uint32_t i = g.orig[p];
+        if (par[i] != SG_NONE) { g.tpar[p] = g.pos[par[i]]; g.teid[p] = par_e[i]; }
     }
-    for (uint32_t k = 0; k < K; ++k) { g.cls[k].slice0 = g.cls[k].pos0 / 32; g.cls[k].nslices = g.cls[k].n / 32; }
-    const uint64_t entries = 32ull * g.slice_ptr[nslices];
-    g.col.resize(entries); g.eid.assign(entries, SG_NONE);
-    g.entry_of_edge.assign(M, 0);
-    const bool sort_rows = std::getenv("SG_VB_ROWS") == nullptr || std::strcmp(std::getenv("SG_VB_ROWS"), "edge") != 0;   // measurement knob
-    for (uint64_t s = 0; s < nslices; ++s) {
-        const uint64_t base = 32ull * g.slice_ptr[s];
-        const uint32_t D = g.slice_ptr[s + 1] - g.slice_ptr[s];
-        for (uint32_t j = 0; j < 32; ++j) {
-            const uint64_t p = 32 * s + j;
-            const uint32_t i = g.orig[p];
-            const uint32_t d = g.deg[p];
-            // a row lists its neighbours by ascending position (= by class, then by BFS index): the 32 sites of a
-            // slice are close in BFS index, so their k-th neighbours tend to share 128-byte lines
-            uint64_t key[32];
-            if (i != SG_NONE) {
-                const uint64_t r0 = g.row_ptr[i];
-                for (uint32_t q = 0; q < d; ++q) key[q] = (uint64_t)g.pos[g.adj[r0 + q]] << 32 | g.adj_e[r0 + q];
-                if (sort_rows) std::sort(key, key + d);
-            }
-            for (uint32_t q = 0; q < D; ++q) {
-                const uint64_t ent = base + 32ull * q + j;
-                if (i != SG_NONE && q < d) {
-                    g.col[ent] = (uint32_t)(key[q] >> 32);
-                    const uint32_t e = (uint32_t)key[q];
-                    g.eid[ent] = e;
-                    if (g.eu[e] == i) g.entry_of_edge[e] = (uint32_t)ent;
-                } else {
-                    g.col[ent] = (uint32_t)p;   // padding entry: points at its own position, coupling word 0
+    // slices: greedy runs of <= 32 positions of one class within the entry budget
+    g.hdr.clear(); g.orig_s.clear(); g.rp_s.clear();
+    g.col.clear(); g.col.reserve(2 * M); g.jeid.clear();
+    std::vector<uint32_t> rowT, rowX;            // the slice's X entries are appended after its T entries
+    std::vector<uint32_t> rowXe;
+    for (uint32_t k = 0; k < K; ++k) {
+        g.cls[k].slice0 = g.hdr.size();
+        uint64_t p = g.cls[k].pos0;
+        const uint64_t pend = p + g.cls[k].n;
+        while (p < pend) {
+            SGHdr h{(uint32_t)p, (uint32_t)g.col.size(), (uint32_t)g.jeid.size(), 0u};
+            uint32_t n = 0, sT = 0, sX = 0;
+            rowT.clear(); rowX.clear(); rowXe.clear();
+            const size_t base = g.orig_s.size();
+            g.orig_s.resize(base + 32, SG_NONE); g.rp_s.resize(base + 32, 0u);
+            while (p < pend && n < 32) {
+                const uint32_t i = g.orig[p];
+                const uint32_t d = (uint32_t)(g.row_ptr[i + 1] - g.row_ptr[i]), t = nT[i], x = d - t;
+                if (n > 0 && (sT + t > g.cap || sX + x > g.cap)) break;
+                // tree entries: parent first, then children by position; other entries by position
+                uint64_t keyT[32], keyX[32];
+                uint32_t cT = 0, cX = 0;
+                for (uint64_t a = g.row_ptr[i]; a < g.row_ptr[i + 1]; ++a) {
+                    const uint32_t v = g.adj[a], e = g.adj_e[a];
+                    const uint64_t key = (uint64_t)g.pos[v] << 32 | e;
+                    if (g.gauge && par_e[i] == e) { std::memmove(keyT + 1, keyT, cT * sizeof(uint64_t)); keyT[0] = key; cT++; }
+                    else if (g.gauge && par_e[v] == e) keyT[cT++] = key;
+                    else keyX[cX++] = key;
                 }
+                std::sort(keyT + ((g.gauge && par_e[i] != SG_NONE) ? 1 : 0), keyT + cT);
+                std::sort(keyX, keyX + cX);
+                g.orig_s[base + n] = i;
+                g.rp_s[base + n] = sT | sX << 10 | cT << 20 | cX << 25;
+                for (uint32_t q = 0; q < cT; ++q) rowT.push_back((uint32_t)(keyT[q] >> 32));
+                for (uint32_t q = 0; q < cX; ++q) { rowX.push_back((uint32_t)(keyX[q] >> 32)); rowXe.push_back((uint32_t)keyX[q]); }
+                sT += cT; sX += cX; ++n; ++p;
             }
+            h.counts = n | sT << 6 | sX << 16;
+            g.hdr.push_back(h);
+            g.col.insert(g.col.end(), rowT.begin(), rowT.end());
+            g.col.insert(g.col.end(), rowX.begin(), rowX.end());
+            g.jeid.insert(g.jeid.end(), rowXe.begin(), rowXe.end());
+            if (g.col.size() >= (1ull << 32)) { sg_set_error("sg_create: instance too large for 32-bit entry indices"); return false; }
         }
+        g.cls[k].nslices = g.hdr.size() - g.cls[k].slice0;
     }
+    g.hdr.push_back(SGHdr{(uint32_t)N, (uint32_t)g.col.size(), (uint32_t)g.jeid.size(), 0u});
     return true;
 }
+
+// Entry budget of a slice: its T and X entries are parked in shared memory (8 bytes per entry and word of the group):
+// 2 KiB per warp at one word per thread, 4 KiB at two or four.
+uint32_t sg_vb_slice_cap(uint32_t n_words) { return n_words % 4 ? 128u : 64u; }
 
 // ---- host-only C entry points (include/sg.h) ------------------------------------------------------
 struct sg_host_graph { VBHostGraph g; };
@@ -299,12 +310,13 @@ extern "C" void sg_host_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c
     for (int q = 0; q < 4; ++q) out[q] = x.x[q];
 }
 
-extern "C" sg_host_graph *sg_host_graph_create(int model, uint64_t N, double c, uint64_t seed)
+extern "C" sg_host_graph *sg_host_graph_create(int model, uint64_t N, double c, uint64_t seed, uint32_t n_words)
 {
     if (model != SG_MODEL_VB && model != SG_MODEL_RRBG) { sg_set_error("sg_host_graph_create: graph model required"); return nullptr; }
-    if (N < 2 || N >= (1ull << 32)) { sg_set_error("sg_host_graph_create: N must satisfy 2 <= N < 2^32"); return nullptr; }
+    if (N < 2 || N >= (1ull << 31) - 2) { sg_set_error("sg_host_graph_create: N must satisfy 2 <= N < 2^31 - 2"); return nullptr; }
+    if (n_words == 0) { sg_set_error("sg_host_graph_create: n_words must be >= 1"); return nullptr; }
     sg_host_graph *h = new sg_host_graph();
-    if (!sg_build_vb_graph(model, N, c, seed, h->g)) { delete h; return nullptr; }
+    if (!sg_build_vb_graph(model, N, c, seed, n_words, h->g)) { delete h; return nullptr; }
     return h;
 }
 
@@ -313,14 +325,16 @@ extern "C" void sg_host_graph_destroy(sg_host_graph *g) { delete g; }
 extern "C" int sg_host_graph_info(const sg_host_graph *h, uint64_t *info)
 {
     if (!h || !info) return SG_EINVAL;
-    info[0] = h->g.M; info[1] = h->g.K; info[2] = h->g.dmax; info[3] = h->g.col.size();
-    info[4] = h->g.slice_ptr.size() - 1; info[5] = h->g.N; info[6] = h->g.P; info[7] = SG_SORT_WINDOW;
+    const VBHostGraph &g = h->g;
+    info[0] = g.M; info[1] = g.K; info[2] = g.dmax; info[3] = g.col.size();
+    info[4] = g.hdr.size() - 1; info[5] = g.N; info[6] = g.jeid.size(); info[7] = g.cap; info[8] = g.gauge ? 1 : 0;
     return SG_OK;
 }
 
 extern "C" int sg_host_graph_get(const sg_host_graph *h, uint32_t *u, uint32_t *v, uint32_t *colour, uint32_t *orig,
-                                 uint32_t *deg, uint32_t *slice_ptr, uint32_t *col, uint32_t *eid,
-                                 uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0)
+                                 uint32_t *hdr, uint32_t *orig_s, uint32_t *rp_s, uint32_t *col, uint32_t *jeid,
+                                 uint32_t *tpar, uint32_t *teid, uint32_t *bfs_pos,
+                                 uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0, uint64_t *class_nslices)
 {
     if (!h) return SG_EINVAL;
     const VBHostGraph &g = h->g;
@@ -328,14 +342,19 @@ extern "C" int sg_host_graph_get(const sg_host_graph *h, uint32_t *u, uint32_t *
     if (v) std::copy(g.ev.begin(), g.ev.end(), v);
     if (colour) std::copy(g.colour.begin(), g.colour.end(), colour);
     if (orig) std::copy(g.orig.begin(), g.orig.end(), orig);
-    if (deg) std::copy(g.deg.begin(), g.deg.end(), deg);
-    if (slice_ptr) std::copy(g.slice_ptr.begin(), g.slice_ptr.end(), slice_ptr);
+    if (hdr) std::memcpy(hdr, g.hdr.data(), g.hdr.size() * sizeof(SGHdr));
+    if (orig_s) std::copy(g.orig_s.begin(), g.orig_s.end(), orig_s);
+    if (rp_s) std::copy(g.rp_s.begin(), g.rp_s.end(), rp_s);
     if (col) std::copy(g.col.begin(), g.col.end(), col);
-    if (eid) std::copy(g.eid.begin(), g.eid.end(), eid);
+    if (jeid) std::copy(g.jeid.begin(), g.jeid.end(), jeid);
+    if (tpar) std::copy(g.tpar.begin(), g.tpar.end(), tpar);
+    if (teid) std::copy(g.teid.begin(), g.teid.end(), teid);
+    if (bfs_pos) std::copy(g.bfs_pos.begin(), g.bfs_pos.end(), bfs_pos);
     for (uint32_t k = 0; k < g.K; ++k) {
         if (class_pos0) class_pos0[k] = g.cls[k].pos0;
         if (class_n) class_n[k] = g.cls[k].n;
         if (class_slice0) class_slice0[k] = g.cls[k].slice0;
+        if (class_nslices) class_nslices[k] = g.cls[k].nslices;
     }
     return SG_OK;
 }

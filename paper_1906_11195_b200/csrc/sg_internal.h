@@ -22,72 +22,93 @@ struct Philox4 { uint32_t x[4]; };
 Philox4 sg_philox_host(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1);
 
 // ---- VB instance layout -----------------------------------------------------------------------
-// Sites are relabelled to "positions" p: class-major (colour 0, 1, ...), every class starting at a multiple of
-// 32 (gap positions are padding: orig = SG_NONE, spin word 0, never written).  Inside a class the sites keep
-// their breadth-first index order (the locality-improving relabelling), except that every window of
-// SG_SORT_WINDOW consecutive sites is stably sorted by degree.  Slice g = positions 32g..32g+31 stores its rows
-// column-major (sliced ELL) with row length D_g = the largest degree in the slice: the k-th neighbour of the
-// j-th site of the slice lives at index 32*slice_ptr[g] + 32*k + j of `col` (neighbour position) and, times
-// n_words plus w, of the coupling array.  Entries beyond a site's degree (and all entries of padding positions)
-// point at the site's own position with coupling word 0.
+// Sites are relabelled to "positions" p = 0..N-1: class-major (colour 0, 1, ...), and inside a class in
+// breadth-first index order (BFS over the whole graph, roots in label order, rows in edge order): the
+// locality-improving relabelling.  It is free: the order inside a colour class changes no output (Q15).
+// Gauge fixing: the breadth-first forest's edges carry J = +1 in every lane after the transformation
+// s_i -> eps_i s_i, J_ij -> eps_i J_ij eps_j with eps_child = eps_parent * J_(parent,child) (eps_root = +1), which
+// changes no bond state, hence no flip decision, energy or correlation count.  The device stores the
+// transformed spins and couplings; tree entries ("T") need no coupling word at all, the others ("X") do.
+// A class is cut into slices: runs of at most 32 consecutive positions with at most `cap` T entries and at most
+// `cap` X entries in total (cap >= 31, so a single site always fits).  A slice is one warp's work:
+//   hdr[g]           = first position, first index in `col`, first index in the coupling array, and
+//                      n | nTs << 6 | nXs << 16  (sites, T entries, X entries of the slice);
+//   col              = for every slice its T entries in site order (parent first, then children by position), then
+//                      its X entries in site order (by position); the coupling array follows the X order;
+//   orig_s[32 g + j] = original label of the j-th site of slice g (SG_NONE for j >= n): the Philox counter;
+//   rp_s[32 g + j]   = tOff | xOff << 10 | nT << 20 | nX << 25: where the site's T / X entries start inside the
+//                      slice's T / X run, and how many there are.
+// The kernels read a slice's entries with one lane per ENTRY (every lane busy whatever the degrees, streams
+// coalesced, neighbouring entries gather from neighbouring words), park spin ^ coupling in shared memory, and
+// finish with one lane per SITE.
 constexpr uint32_t SG_NONE = 0xFFFFFFFFu;
-constexpr uint32_t SG_SORT_WINDOW = 16384;
 
 struct VBClass {
-    uint64_t pos0;     // first position of the class (multiple of 32)
-    uint64_t n;        // positions in the class, padding included (multiple of 32)
-    uint64_t slice0;   // first slice = pos0 / 32
-    uint64_t nslices;  // n / 32
+    uint64_t pos0;     // first position of the class
+    uint64_t n;        // sites in the class
+    uint64_t slice0;   // first slice
+    uint64_t nslices;
 };
+
+struct alignas(16) SGHdr { uint32_t pos0, col_off, j_off, counts; };
 
 struct VBHostGraph {
     uint64_t N = 0, M = 0;
-    uint64_t P = 0;                        // positions including padding (multiple of 32)
     uint32_t K = 0, dmax = 0;
+    uint32_t cap = 0;                      // entry budget of a slice (T and X each)
+    bool gauge = true;
     std::vector<uint32_t> eu, ev;          // M edges in generation order (original labels)
     std::vector<uint64_t> row_ptr;         // N+1 (original labels)
     std::vector<uint32_t> adj;             // 2M neighbours, rows in increasing edge id
     std::vector<uint32_t> adj_e;           // 2M edge ids
     std::vector<uint8_t> colour;           // N
-    std::vector<uint32_t> orig;            // position -> original label, SG_NONE for padding positions
+    std::vector<uint32_t> orig;            // position -> original label
     std::vector<uint32_t> pos;             // original label -> position
     std::vector<VBClass> cls;              // K classes
-    std::vector<uint32_t> slice_ptr;       // nslices_total+1, units of 32 entries
-    std::vector<uint32_t> col;             // 32*slice_ptr.back() entries: neighbour positions
-    std::vector<uint32_t> eid;             // same length: edge id or 0xFFFFFFFF for padding
-    std::vector<uint8_t> deg;              // per position (padding positions: 0)
-    std::vector<uint32_t> entry_of_edge;   // M: entry index of edge e at endpoint eu[e]
+    std::vector<SGHdr> hdr;                // per slice, plus one sentinel (pos0 = N, offsets = totals, counts = 0)
+    std::vector<uint32_t> orig_s, rp_s;    // 32 per slice
+    std::vector<uint32_t> col;             // 2M neighbour positions
+    std::vector<uint32_t> jeid;            // edge id of every coupling entry
+    std::vector<uint32_t> tpar, teid;      // per position: parent position / tree edge id (SG_NONE: root)
+    std::vector<uint32_t> bfs_pos;         // positions in breadth-first order (parents before children)
 };
 
 // Builds everything above.  Returns false and sets the error string on bad arguments.
-bool sg_build_vb_graph(int model /* SG_MODEL_VB or SG_MODEL_RRBG */, uint64_t N, double c, uint64_t seed, VBHostGraph &g);
+bool sg_build_vb_graph(int model /* SG_MODEL_VB or SG_MODEL_RRBG */, uint64_t N, double c, uint64_t seed, uint32_t n_words, VBHostGraph &g);
+uint32_t sg_vb_slice_cap(uint32_t n_words);   // entry budget of a slice for this number of words per site
 
 std::vector<uint64_t> sg_vb_thresholds(double T, uint32_t dmax);   // thr[0..dmax], thr[0]=0
 std::vector<uint64_t> sg_sk_thresholds(double T, uint64_t N);      // thr[0..N-1]
 
 // ---- device launchers (sg_kernels.cu) ---------------------------------------------------------
 struct VBDevice {
-    uint64_t *spin = nullptr;       // P*W words, position-major word-minor
-    uint64_t *J = nullptr;          // entries*W coupling words
-    uint32_t *col = nullptr;        // entries
-    uint32_t *orig = nullptr;       // P (SG_NONE = padding)
-    uint32_t *slice_ptr = nullptr;  // nslices+1
-    uint64_t *thr = nullptr;        // 32 thresholds (thr[k], k=0..31; beyond dmax = 0)
+    uint64_t *spin = nullptr;       // N*W words, position-major word-minor, gauge-transformed (sigma ^ eps)
+    uint64_t *eps = nullptr;        // N*W words: the gauge (all 0 without gauge fixing); getters/setters only
+    uint64_t *J = nullptr;          // nJ*W transformed coupling words (X entries only)
+    uint32_t *col = nullptr;        // neighbour positions
+    uint32_t *orig = nullptr;       // N: position -> label (getters / setters)
+    uint32_t *orig_s = nullptr;     // 32 per slice
+    uint32_t *rp_s = nullptr;       // 32 per slice
+    SGHdr *hdr = nullptr;           // nslices+1
+    uint32_t nslices = 0, cap = 0;
+    uint64_t thr_host[32] = {0};    // thresholds thr[k], k=0..31 (beyond dmax = 0): passed to the kernels by value
 };
 
 struct SGSeed { uint32_t k0, k1; };
 
-int sgk_init_spins(uint64_t *spin, const uint32_t *orig, uint64_t N, uint32_t W, SGSeed key, cudaStream_t st);
-int sgk_init_vb_couplings(uint64_t *J, const uint32_t *eid, uint64_t entries, uint32_t W, SGSeed key, cudaStream_t st);
-// one colour class of one sweep; P, entries = sizes of the whole instance (choose 32- or 64-bit index arithmetic);
+int sgk_init_spins(uint64_t *spin, const uint32_t *orig, const uint64_t *eps, uint64_t N, uint32_t W, SGSeed key, cudaStream_t st);
+// draws every coupling entry (O3) and applies the gauge; jeid: device, edge id per coupling entry
+int sgk_init_vb_couplings(const VBDevice &d, const uint32_t *jeid, uint32_t W, SGSeed key, cudaStream_t st);
+// one colour class of one sweep; N, nJ = sizes of the whole instance (choose 32- or 64-bit index arithmetic);
 // reverse = walk the class from its last slice to its first (callers alternate it from launch to launch)
-int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint64_t P, uint64_t entries, uint32_t W, uint64_t sweep, SGSeed key,
+int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint64_t N, uint64_t nJ, uint32_t W, uint64_t sweep, SGSeed key,
                        bool reverse, cudaStream_t st);
 // counts[64*W] (device, u64) += per-lane number of set bits of (a XOR b) over n_sites*W words
 int sgk_xor_popcount(const uint64_t *a, const uint64_t *b, uint64_t n_sites, uint32_t W, uint64_t *counts, cudaStream_t st);
-// counts[64*W] += per-lane sum over the class's sites of u_i (unsatisfied incident bonds)
-int sgk_vb_unsat_class(const VBDevice &d, const VBClass &c, uint32_t W, uint64_t *counts, cudaStream_t st);
-int sgk_permute_words(const uint64_t *src, uint64_t *dst, const uint32_t *map, uint64_t N, uint32_t W, bool scatter, cudaStream_t st);
+// counts[64*W] += per-lane sum over all sites of u_i (unsatisfied incident bonds): one launch over the whole instance
+int sgk_vb_unsat(const VBDevice &d, uint64_t N, uint64_t nJ, uint32_t W, uint64_t *counts, cudaStream_t st);
+int sgk_permute_words(const uint64_t *src, uint64_t *dst, const uint32_t *map, const uint64_t *eps, uint64_t N, uint32_t W, bool scatter,
+                      cudaStream_t st);
 
 // SK
 struct SKDevice {

@@ -21,7 +21,7 @@ struct sg_sim {
     VBDevice vb;
     std::vector<uint64_t> thr_host;
     bool vb_reverse = false;                 // direction of the next colour-class launch (alternates)
-    uint64_t vb_entries = 0;                 // sliced-ELL entries (padding included)
+    uint64_t vb_nJ = 0;                      // coupling entries
     // SK
     SKDevice sk;
     // common

@@ -47,6 +47,10 @@ def _assert_same_state(g, o):
     (300, 0.0, 1.0, 7, 1),       # no edges: every site flips every sweep
     (512, 12.0, 2.0, 8, 1),      # dense: degrees up to ~25, several chunks of 4 neighbours
     (640, 4.0, 1.0, 9, 16),      # W=16 (config 5's small sizes)
+    (300, 4.0, 1.0, 10, 64),     # W=64: 16 word groups of four; counts beyond 32 words
+    (500, 5.0, 1.4, 11, 33),     # W=33: odd word count above 32 (one-word kernel with 33 groups, strided count kernels)
+    (900, 4.0, 0.6, 12, 6),      # W=6: word groups of two
+    (2000, 14.0, 1.0, 13, 1),    # mean degree 14: every slice is cut short by the entry budget, long rows in phase 2
 ])
 def test_instance_and_first_sweeps_match(sg, oracle_mod, N, c, T, seed, W):
     g, o = _pair(sg, oracle_mod, N, c, T, seed, W)
@@ -59,14 +63,32 @@ def test_instance_and_first_sweeps_match(sg, oracle_mod, N, c, T, seed, W):
     assert np.array_equal(g.thresholds(g.max_degree + 1), o.thresholds(o.max_degree + 1))
     _assert_same_state(g, o)
     assert np.array_equal(g.energy(), o.energy())
+    g.snapshot(2); o.snapshot(2)
     for _ in range(6):
         g.sweep(1)
         o.sweep(1)
         _assert_same_state(g, o)
         assert np.array_equal(g.energy(), o.energy())
+        assert np.array_equal(g.correlation(2), o.correlation(2))
     g.sweep(5)
     o.sweep(5)
     _assert_same_state(g, o)
+    assert np.array_equal(g.correlation(2), o.correlation(2))
+
+
+@pytest.mark.parametrize("N,c,T,seed,W", [(3000, 4.0, 1.0, 31, 1), (1500, 6.0, 0.6, 32, 4), (800, 4.0, 1.4, 33, 3), (700, 4.0, 1.0, 34, 2)])
+def test_wide_index_path(sg, oracle_mod, monkeypatch, N, c, T, seed, W):
+    """The 64-bit index instantiations of the sweep and energy kernels (taken when N*W or the coupling array reaches
+    2^32 words, e.g. N = 2^26 with W >= 16) forced on small instances with the test knob SG_FORCE_WIDE."""
+    monkeypatch.setenv("SG_FORCE_WIDE", "1")
+    g, o = _pair(sg, oracle_mod, N, c, T, seed, W)
+    g.snapshot(0); o.snapshot(0)
+    for _ in range(4):
+        g.sweep(2)
+        o.sweep(2)
+        _assert_same_state(g, o)
+        assert np.array_equal(g.energy(), o.energy())
+        assert np.array_equal(g.correlation(0), o.correlation(0))
 
 
 def test_config1_full_protocol(sg, oracle_mod):
@@ -207,73 +229,96 @@ def _lane_counts(x):
     return out
 
 
-@pytest.mark.parametrize("T", [1.0, 0.6])
-def test_full_size_config3_late_sweep(sg, oracle_mod, T):
-    """BASELINE.json configs[2] at full size (N = 2^24, W = 1, T = 1 and 0.6), in the launch configuration bench.py times:
-    the GPU runs 40 sweeps, then ONE more sweep is compared element by element with the oracle started from the
-    GPU's state at sweep 40 (a sweep is a pure function of (state, index), Q15), together with the
-    correlation counts against a snapshot and the energy change (oracle's accumulated dE of that sweep)."""
-    N, W, T0 = 1 << 24, 1, 40
-    g = sg.Sim(sg.SG_MODEL_VB, N, 4.0, T, 1, W)
-    o = oracle_mod.Oracle(oracle_mod.VB, N, 4.0, T, 1, W)
-    assert g.M == o.M and g.n_colours == o.n_colours and g.max_degree == o.max_degree
-    assert np.array_equal(g.spins(), o.spins())                   # initial configuration
-    idx = np.random.default_rng(1).integers(0, g.M, size=200000)
-    assert np.array_equal(g.couplings()[idx], o.couplings()[idx])
-    g.sweep(T0)
+def _threads(fns):
+    """Run callables concurrently (the oracle's C calls release the GIL) and return their results in order."""
+    from concurrent.futures import ThreadPoolExecutor
+
+    with ThreadPoolExecutor(max_workers=len(fns)) as ex:
+        return [f.result() for f in [ex.submit(fn) for fn in fns]]
+
+
+def _late_sweep_check(g, o, t):
+    """One sweep compared element by element at sweep index t: the oracle restarts from the GPU's state (a sweep is a
+    pure function of (state, index), Q15); also the energy change (the oracle's accumulated dE of that
+    sweep) and the correlation counts against a snapshot taken before the sweep."""
+    assert g.sweep_count == t
     before = g.spins()
     E_before = g.energy()
     g.snapshot(0)
     o.set_spins(before)
-    o.set_sweep_count(T0)
+    o.set_sweep_count(t)
     dE0 = o.accumulated_dE().copy()
     g.sweep(1)
     o.sweep(1)
     after = g.spins()
-    assert np.array_equal(after, o.spins())
+    assert np.array_equal(after, o.spins()), f"sweep index {t}"
     assert np.array_equal(g.energy() - E_before, o.accumulated_dE() - dE0)
     assert np.array_equal(g.correlation(0), _lane_counts(before ^ after))
 
 
-def test_config2_full_size_first_sweeps(sg, oracle_mod):
-    """BASELINE.json configs[1] at full size: N = 2^20, 4 words (256 samples) per site."""
+def test_full_size_config3(sg, oracle_mod):
+    """BASELINE.json configs[2] at full size (N = 2^24, W = 1, T = 0.6, 1.0, 1.4), in the launch configuration
+    bench.py times, following SURVEY.md 8(c)'s parity protocol: the instance (initial spins, sampled couplings), the
+    first sweeps in full (4 at T = 1.0, 2 at the other temperatures), then the LAST sweep of the 4096-sweep run,
+    index t = S - 1 = 4095, compared element by element.  The three oracles run in parallel threads."""
+    N, W, S = 1 << 24, 1, 1 << 12
+    Ts = (1.0, 0.6, 1.4)
+    first = {1.0: 4, 0.6: 2, 1.4: 2}
+    os_ = _threads([lambda T=T: oracle_mod.Oracle(oracle_mod.VB, N, 4.0, T, 1, W) for T in Ts])
+    gs = [sg.Sim(sg.SG_MODEL_VB, N, 4.0, T, 1, W) for T in Ts]
+    g0, o0 = gs[0], os_[0]
+    assert g0.M == o0.M and g0.n_colours == o0.n_colours and g0.max_degree == o0.max_degree
+    idx = np.random.default_rng(1).integers(0, g0.M, size=200000)
+    assert np.array_equal(g0.couplings()[idx], o0.couplings()[idx])
+
+    def run(g, o, T):
+        assert np.array_equal(g.spins(), o.spins())                   # initial configuration
+        for t in range(first[T]):
+            g.sweep(1)
+            o.sweep(1)
+            assert np.array_equal(g.spins(), o.spins()), (T, t)
+        assert np.array_equal(g.energy(), o.energy())
+        g.sweep(S - 1 - first[T])
+        _late_sweep_check(g, o, S - 1)
+        return True
+
+    assert all(_threads([lambda g=g, o=o, T=T: run(g, o, T) for g, o, T in zip(gs, os_, Ts)]))
+
+
+def test_config2_full_size(sg, oracle_mod):
+    """BASELINE.json configs[1] at full size: N = 2^20, 4 words (256 samples) per site: the first sweeps in full and a
+    late sweep."""
     N, W = 1 << 20, 4
     g, o = _pair(sg, oracle_mod, N, 4.0, 1.0, 1, W)
-    g.snapshot(0); o.snapshot(0)
+    g.snapshot(1); o.snapshot(1)
     for _ in range(2):
         g.sweep(1)
         o.sweep(1)
         _assert_same_state(g, o)
-    assert np.array_equal(g.correlation(0), o.correlation(0))
+    assert np.array_equal(g.correlation(1), o.correlation(1))
     assert np.array_equal(g.energy(), o.energy())
+    g.sweep(998)
+    _late_sweep_check(g, o, 1000)
 
 
-@pytest.mark.parametrize("T", [float("inf")])     # T = 0 at this size costs another minute of host graph generation; T = 0 is checked at N = 3000
-def test_largest_size_properties(sg, T):
-    """BASELINE.json configs[4] top size N = 2^26 (W = 1), where the oracle is too slow to run in a test: properties
-    that hold at any size.  T = inf: every proposal is accepted, so D alternates N, 0 and the energy is invariant (Q21);
-    T = 0: the energy never increases; always E = M (mod 2); sg_sweep(a); sg_sweep(b) = sg_sweep(a + b)."""
-    N = 1 << 26
-    g = sg.Sim(sg.SG_MODEL_VB, N, 4.0, T, 3, 1)
-    assert g.M == 2 * N
+def test_largest_size_config5(sg, oracle_mod):
+    """BASELINE.json configs[4] top size, N = 2^26 (W = 1) at a finite temperature, with the seed of workloads.cfg5():
+    initial configuration, then one late sweep against the oracle element by element (every word, the energy change,
+    the correlation counts), plus properties that hold at any size (E = M mod 2, D <= N, composition of sweeps)."""
+    from paper_1906_11195_b200.workloads import cfg5
+
+    w = next(x for x in cfg5() if x.N == 1 << 26 and x.T == 1.0)
+    o, g = _threads([lambda: oracle_mod.Oracle(w.model, w.N, w.c, w.T, w.seed, w.n_words),
+                     lambda: sg.Sim(w.model, w.N, w.c, w.T, w.seed, w.n_words)])
+    assert g.M == o.M == 2 * w.N and g.n_colours == o.n_colours and g.max_degree == o.max_degree
+    assert np.array_equal(g.spins(), o.spins())
     E0 = g.energy()
     assert np.all((E0 - g.M) % 2 == 0)
-    g.snapshot(0)
-    g.sweep(1)
-    E1 = g.energy()
-    D1 = g.correlation(0)
-    g.sweep(2)
-    E3 = g.energy()
-    D3 = g.correlation(0)
-    assert np.all((E3 - g.M) % 2 == 0)
-    if math.isinf(T):
-        assert np.array_equal(E1, E0) and np.array_equal(E3, E0)
-        assert np.all(D1 == N) and np.all(D3 == N)
-    else:
-        assert np.all(E1 <= E0) and np.all(E3 <= E1)
-        assert np.all(D1 <= N) and np.all(D1 > 0)
-        # per-lane energy of a random +-J configuration is ~0 +- sqrt(M); a T=0 quench lowers it by O(N)
-        assert np.all(E3 < -0.5 * N)
+    g.sweep(2); g.sweep(3)
+    _late_sweep_check(g, o, 5)
+    D = g.correlation(0)
+    assert np.all(D <= w.N) and np.all(D > 0)
+    assert np.all((g.energy() - g.M) % 2 == 0)
 
 
 @pytest.mark.parametrize("N,T,seed,W", [(1024, 1.2149, 1, 1), (8, 1.0, 2, 1), (4102, 0.6, 3, 2), (1 << 16, 1.2149, 4, 1)])
@@ -298,22 +343,11 @@ def test_rrbg_full_size_late_sweep(sg, oracle_mod):
     """The paper's workload at N = 2^24 (W = 1, T = 0.8 Tc): one late sweep against the oracle, element by element."""
     from paper_1906_11195_b200.workloads import PAPER_RRBG as w
 
-    g = sg.Sim(w.model, w.N, w.c, w.T, w.seed, w.n_words)
-    o = oracle_mod.Oracle(oracle_mod.RRBG, w.N, w.c, w.T, w.seed, w.n_words)
+    o, g = _threads([lambda: oracle_mod.Oracle(oracle_mod.RRBG, w.N, w.c, w.T, w.seed, w.n_words),
+                     lambda: sg.Sim(w.model, w.N, w.c, w.T, w.seed, w.n_words)])
     assert np.array_equal(g.spins(), o.spins())
     g.sweep(30)
-    before = g.spins()
-    E_before = g.energy()
-    g.snapshot(0)
-    o.set_spins(before)
-    o.set_sweep_count(30)
-    dE0 = o.accumulated_dE().copy()
-    g.sweep(1)
-    o.sweep(1)
-    after = g.spins()
-    assert np.array_equal(after, o.spins())
-    assert np.array_equal(g.energy() - E_before, o.accumulated_dE() - dE0)
-    assert np.array_equal(g.correlation(0), _lane_counts(before ^ after))
+    _late_sweep_check(g, o, 30)
 
 
 def test_windowed_protocol_matches_oracle(sg, oracle_mod):

@@ -46,7 +46,7 @@ def test_no_cpu_fallback(sg):
 def test_bad_arguments_are_rejected_before_touching_the_gpu(sg):
     for args in [(7, 100, 4.0, 1.0, 1, 1), (0, 1, 4.0, 1.0, 1, 1), (0, 100, 4.0, 1.0, 1, 0),
                  (0, 100, 4.0, -0.5, 1, 1), (0, 100, 4.0, float("nan"), 1, 1), (1, 40000, 0.0, 1.0, 1, 1),
-                 (0, 1 << 31, 4.0, 1.0, 1, 1), (2, 1001, 0.0, 1.0, 1, 1), (2, 6, 0.0, 1.0, 1, 1)]:
+                 (0, (1 << 31) - 2, 4.0, 1.0, 1, 1), (2, 1001, 0.0, 1.0, 1, 1), (2, 6, 0.0, 1.0, 1, 1)]:
         with pytest.raises(sg.SGError):
             sg.Sim(*args)
 
@@ -61,98 +61,194 @@ def test_host_philox_known_answers(sg):
         assert list(binding.host_philox(*v[:6])) == v[6:]
 
 
-@pytest.mark.parametrize("model,N,c,seed", [(0, 1024, 4.0, 1), (0, 5000, 4.0, 77), (0, 333, 2.5, 3), (0, 64, 7.0, 5), (0, 100, 0.0, 1),
-                                            (2, 8, 0.0, 1), (2, 1024, 0.0, 2), (2, 4102, 0.0, 3)])
-def test_host_generator_matches_oracle_and_layout_is_consistent(sg, oracle_mod, model, N, c, seed):
-    """model 0: Erdos-Renyi (O2); model 2: random regular bipartite graph of degree 4 (O2b)."""
+def _bfs_forest(N, e):
+    """Breadth-first forest over the whole graph, roots in label order, rows in edge order: order, parent, parent edge."""
+    rows = [[] for _ in range(N)]
+    for k, (a, b) in enumerate(e.astype(np.int64).tolist()):
+        rows[a].append((b, k)); rows[b].append((a, k))
+    order, par, par_e, seen = [], [-1] * N, [-1] * N, np.zeros(N, dtype=bool)
+    for r in range(N):
+        if seen[r]:
+            continue
+        seen[r] = True
+        order.append(r)
+        head = len(order) - 1
+        while head < len(order):
+            u_ = order[head]
+            for v_, k in rows[u_]:
+                if not seen[v_]:
+                    seen[v_] = True
+                    par[v_], par_e[v_] = u_, k
+                    order.append(v_)
+            head += 1
+    return rows, order, par, par_e
+
+
+def _decode_rows(g):
+    """Walk the slices exactly as the kernels do: per position the tree list, the other list (neighbour position,
+    coupling-entry index), and the label the slice carries for the site."""
+    N = g["N"]
+    T = [[] for _ in range(N)]
+    X = [[] for _ in range(N)]
+    label = np.full(N, -1, dtype=np.int64)
+    hdr = g["hdr"].astype(np.int64)
+    for s_ in range(g["nslices"]):
+        pos0, col_off, j_off, counts = hdr[s_]
+        n, nTs, nXs = counts & 63, (counts >> 6) & 1023, counts >> 16
+        assert 1 <= n <= 32 and nTs <= g["cap"] and nXs <= g["cap"]
+        assert hdr[s_ + 1][1] == col_off + nTs + nXs and hdr[s_ + 1][2] == j_off + nXs
+        t_run, x_run = 0, 0
+        for j in range(32):
+            rp = int(g["rp_s"][32 * s_ + j])
+            if j >= n:
+                assert g["orig_s"][32 * s_ + j] == 0xFFFFFFFF and rp == 0
+                continue
+            p = pos0 + j
+            label[p] = int(g["orig_s"][32 * s_ + j])
+            tOff, xOff, nT, nX = rp & 1023, (rp >> 10) & 1023, (rp >> 20) & 31, rp >> 25
+            assert tOff == t_run and xOff == x_run                 # site order, no gaps
+            T[p] = [int(q) for q in g["col"][col_off + tOff:col_off + tOff + nT]]
+            X[p] = [(int(g["col"][col_off + nTs + xOff + r]), int(j_off + xOff + r)) for r in range(nX)]
+            t_run += nT; x_run += nX
+        assert t_run == nTs and x_run == nXs
+    return T, X, label
+
+
+@pytest.mark.parametrize("model,N,c,seed,W", [(0, 1024, 4.0, 1, 1), (0, 5000, 4.0, 77, 4), (0, 333, 2.5, 3, 1), (0, 64, 7.0, 5, 2), (0, 100, 0.0, 1, 1),
+                                              (0, 3000, 14.0, 9, 1), (2, 8, 0.0, 1, 1), (2, 1024, 0.0, 2, 1), (2, 4102, 0.0, 3, 16)])
+def test_host_generator_matches_oracle_and_layout_is_consistent(sg, oracle_mod, model, N, c, seed, W):
+    """model 0: Erdos-Renyi (O2); model 2: random regular bipartite graph of degree 4 (O2b).  The layout rules of
+    include/sg.h (sg_host_graph_*) are re-derived here in plain Python from the oracle's edge list and colouring."""
     from paper_1906_11195_b200 import binding
 
-    g = binding.host_graph(N, c, seed, model)
+    g = binding.host_graph(N, c, seed, model, W)
     o = oracle_mod.Oracle(model, N, c, 1.0, seed, 1)
     assert g["M"] == o.M and g["K"] == o.n_colours and g["dmax"] == o.max_degree
     e = o.edges()
     assert np.array_equal(g["u"], e[:, 0]) and np.array_equal(g["v"], e[:, 1])
     _, _, colour = o.graph()
     assert np.array_equal(g["colour"], colour)
-    # positions: class-major; inside a class the valid positions are the class's sites in breadth-first order
-    # (roots in label order, rows in edge order), each window of sort_window sites stably sorted by degree;
-    # classes start at multiples of 32, gaps are padding (orig = NONE)
     NONE = 0xFFFFFFFF
-    P = g["P"]
-    assert P % 32 == 0 and g["nslices"] == P // 32
-    orig_all = g["orig"].astype(np.int64)
-    valid = orig_all != NONE
-    orig = orig_all[valid]
+    K, cap = g["K"], g["cap"]
+    assert g["gauge"] == 1 and cap == (64 if W % 4 == 0 else 128)
+    orig = g["orig"].astype(np.int64)
     assert np.array_equal(np.sort(orig), np.arange(N))
-    degree = np.bincount(e.ravel().astype(np.int64), minlength=N)
-    assert np.array_equal(g["deg"][valid], degree[orig]) and np.all(g["deg"][~valid] == 0)
-    rows = [[] for _ in range(N)]
-    for a, b in e.astype(np.int64).tolist():
-        rows[a].append(b); rows[b].append(a)
-    bfs, seen = [], np.zeros(N, dtype=bool)
-    for r in range(N):
-        if seen[r]:
-            continue
-        seen[r] = True
-        bfs.append(r)
-        head = len(bfs) - 1
-        while head < len(bfs):
-            for v_ in rows[bfs[head]]:
-                if not seen[v_]:
-                    seen[v_] = True
-                    bfs.append(v_)
-            head += 1
-    SW = g["sort_window"]
-    for k in range(g["K"]):
-        p0, n, s0 = int(g["class_pos0"][k]), int(g["class_n"][k]), int(g["class_slice0"][k])
-        assert p0 % 32 == 0 and n % 32 == 0 and s0 == p0 // 32
-        members = [i for i in bfs if colour[i] == k]
-        assert 0 <= n - len(members) < 32
-        expect = []
-        for w0 in range(0, len(members), SW):
-            expect += sorted(members[w0:w0 + SW], key=lambda i: degree[i])      # sorted() is stable
-        assert orig_all[p0:p0 + len(members)].tolist() == expect
-        assert np.all(orig_all[p0 + len(members):p0 + n] == NONE)
     pos = np.empty(N, dtype=np.int64)
-    pos[orig] = np.nonzero(valid)[0]
-    sp = g["slice_ptr"].astype(np.int64)
-    # row length of a slice = largest degree in it
-    degs = g["deg"].astype(np.int64).reshape(-1, 32)
-    assert np.array_equal(np.diff(sp), degs.max(axis=1))
-    nbrs = [set() for _ in range(P)]
-    for a, b in e.astype(np.int64):
-        nbrs[pos[a]].add(pos[b]); nbrs[pos[b]].add(pos[a])
+    pos[orig] = np.arange(N)
+    degree = np.bincount(e.ravel().astype(np.int64), minlength=N)
+    rows, order, par, par_e = _bfs_forest(N, e)
+    # positions: class-major; breadth-first order inside a class
+    p0 = 0
+    for k in range(K):
+        members = [i for i in order if colour[i] == k]
+        assert int(g["class_pos0"][k]) == p0 and int(g["class_n"][k]) == len(members)
+        assert orig[p0:p0 + len(members)].tolist() == members
+        p0 += len(members)
+    # forest arrays
+    for p in range(N):
+        i = orig[p]
+        if par[i] < 0:
+            assert g["tpar"][p] == NONE and g["teid"][p] == NONE
+        else:
+            assert g["tpar"][p] == pos[par[i]] and g["teid"][p] == par_e[i]
+    assert np.array_equal(g["bfs_pos"], pos[np.array(order, dtype=np.int64)])
+    # rows: T = parent first, then children by position; X = the other neighbours by position; every coupling
+    # entry carries its edge id; every non-tree edge is stored at both endpoints, every tree edge at none
+    T, X, label = _decode_rows(g)
+    assert np.array_equal(label, orig)
     seen_edges = np.zeros(g["M"], dtype=np.int64)
-    for s_ in range(P // 32):
-        D = sp[s_ + 1] - sp[s_]
-        for j in range(32):
-            p = 32 * s_ + j
-            ents = 32 * sp[s_] + 32 * np.arange(D) + j
-            d = int(g["deg"][p])
-            # padding entries (beyond the degree, or a padding position) point at the site itself, no edge
-            assert np.all(g["eid"][ents[d:]] == NONE) and np.all(g["col"][ents[d:]] == p)
-            if orig_all[p] == NONE:
-                assert d == 0
-                continue
-            assert set(g["col"][ents[:d]].tolist()) == nbrs[p] and len(nbrs[p]) == d
-            for q in range(d):
-                ed = int(g["eid"][ents[q]])
-                a, b = int(e[ed, 0]), int(e[ed, 1])
-                assert {pos[a], pos[b]} == {p, int(g["col"][ents[q]])}
-                seen_edges[ed] += 1
-    assert np.all(seen_edges == 2)                      # every edge stored at both endpoints
-    assert g["entries"] == 32 * sp[-1]
+    nT = np.zeros(N, dtype=np.int64)
+    for p in range(N):
+        i = orig[p]
+        children = sorted(pos[v_] for v_, k in rows[i] if par_e[v_] == k and par[v_] == i)
+        assert T[p] == ([pos[par[i]]] if par[i] >= 0 else []) + children
+        nT[p] = len(T[p])
+        tree_edges = {par_e[i]} | {k for v_, k in rows[i] if par_e[v_] == k and par[v_] == i}
+        others = sorted((pos[v_], k) for v_, k in rows[i] if k not in tree_edges)
+        assert [q for q, _ in X[p]] == [q for q, _ in others]
+        for (q, x), (_, k) in zip(X[p], others):
+            assert g["jeid"][x] == k
+            seen_edges[k] += 1
+    is_tree = np.zeros(g["M"], dtype=bool)
+    is_tree[[k for k in par_e if k >= 0]] = True
+    assert np.all(seen_edges[~is_tree] == 2) and np.all(seen_edges[is_tree] == 0)
+    assert g["entries"] == 2 * g["M"] and g["nJ"] == 2 * int((~is_tree).sum())
+    # slices: greedy cut of every class into runs of <= 32 sites within the entry budget, never across classes
+    hdr = g["hdr"].astype(np.int64)
+    s_ = 0
+    for k in range(K):
+        assert int(g["class_slice0"][k]) == s_
+        p, pend = int(g["class_pos0"][k]), int(g["class_pos0"][k]) + int(g["class_n"][k])
+        while p < pend:
+            n = sT = sX = 0
+            while p + n < pend and n < 32:
+                t, x = nT[p + n], degree[orig[p + n]] - nT[p + n]
+                if n > 0 and (sT + t > cap or sX + x > cap):
+                    break
+                sT += t; sX += x; n += 1
+            assert hdr[s_][0] == p and hdr[s_][3] == (n | sT << 6 | sX << 16)
+            p += n; s_ += 1
+        assert int(g["class_nslices"][k]) == s_ - int(g["class_slice0"][k])
+    assert s_ == g["nslices"] and hdr[s_][0] == N
     # no edge inside a colour class (the race-freedom condition of the parallel update, PAPER.md:320)
     assert np.all(colour[e[:, 0]] != colour[e[:, 1]])
 
 
-def test_padding_overhead_is_small(sg):
+def test_gauged_layout_reproduces_the_oracle_sweep(sg, oracle_mod):
+    """The gauge transformation changes no output (include/sg.h): a plain-Python sweep over the device layout, with the
+    transformed spins sigma ^ eps and couplings kappa ^ eps_i ^ eps_j and NO coupling word on tree entries, gives
+    the oracle's configurations once eps is undone.  Pins the host side of the gauge before any kernel runs."""
+    from paper_1906_11195_b200 import binding
+
+    N, c, T_, seed = 600, 4.0, 1.0, 4
+    g = binding.host_graph(N, c, seed, 0)
+    o = oracle_mod.Oracle(0, N, c, T_, seed, 1)
+    kappa = [int(x) for x in o.couplings()[:, 0]]
+    sigma = [int(x) for x in o.spins()[:, 0]]
+    thr = [int(x) for x in o.thresholds(o.max_degree + 1)] + [0] * 40
+    NONE = 0xFFFFFFFF
+    orig = g["orig"].astype(np.int64)
+    eps = [0] * N
+    for p in g["bfs_pos"].tolist():
+        if g["tpar"][p] != NONE:
+            eps[p] = eps[int(g["tpar"][p])] ^ kappa[int(g["teid"][p])]
+    T, X, _ = _decode_rows(g)
+    spin = [sigma[orig[p]] ^ eps[p] for p in range(N)]
+    J = [0] * g["nJ"]
+    for p in range(N):
+        for q, x in X[p]:
+            J[x] = kappa[int(g["jeid"][x])] ^ eps[p] ^ eps[q]
+    M64 = (1 << 64) - 1
+    for t in range(3):
+        for k in range(g["K"]):
+            p0, n = int(g["class_pos0"][k]), int(g["class_n"][k])
+            for p in range(p0, p0 + n):
+                r = int(oracle_mod.philox(int(orig[p]), 0, t, 0, seed & 0xFFFFFFFF, seed >> 32)[0])
+                bonds = [spin[p] ^ spin[q] for q in T[p]] + [spin[p] ^ spin[q] ^ J[x] for q, x in X[p]]
+                d = len(bonds)
+                flip = 0
+                for b in range(64):
+                    u_ = sum((m >> b) & 1 for m in bonds)
+                    kk = d - 2 * u_
+                    if kk <= 0 or r < thr[kk]:
+                        flip |= 1 << b
+                spin[p] ^= flip & M64
+        o.sweep(1)
+        got = np.zeros(N, dtype=np.uint64)
+        for p in range(N):
+            got[orig[p]] = spin[p] ^ eps[p]
+        assert np.array_equal(got, o.spins()[:, 0]), f"sweep {t}"
+
+
+def test_layout_overhead_is_small(sg):
     from paper_1906_11195_b200 import binding
 
     g = binding.host_graph(1 << 18, 4.0, 1)
-    # padding positions: < 32 per class; padding entries: slices that straddle two degrees inside a sort window
-    assert g["P"] - g["N"] < 32 * g["K"]
-    assert g["entries"] <= 1.02 * 2 * g["M"]
+    # no padding entries at all; the forest's N - (number of components) edges carry no coupling word; almost all
+    # slices are full (32 sites): the per-slice arrays hold little more than one slot per site
+    assert g["entries"] == 2 * g["M"]
+    assert g["nJ"] < 0.52 * g["entries"]
+    assert 32 * g["nslices"] < 1.08 * g["N"]
 
 
 def test_schedule_counts():
