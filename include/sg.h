@@ -54,6 +54,30 @@ enum { SG_OK = 0, SG_EINVAL = -1, SG_ENOMEM = -2, SG_ECUDA = -3, SG_ESLOT = -4 }
  */
 sg_sim *sg_create(int model, uint64_t N, double c, double T, uint64_t seed, uint32_t n_words);
 
+/*
+ * sg_create_opt -- sg_create with options (NULL = all defaults = sg_create).
+ *   word0          the handle simulates words word0 .. word0+n_words-1 of the instance (model, N, c, T, seed): every
+ *                  Philox counter that takes a word index takes word0 + w, so that a job can split the words of one
+ *                  instance over several handles / GPUs and reproduce the single-handle run bit for bit (words share only
+ *                  the graph; Q16, Q24).  Must be a multiple of 4; word0 + n_words <= 2^20.
+ *   n_clones       SK only, 1 or 2: "two clones (i.e. replicas with the same couplings)" simulated side by side
+ *                  (PAPER.md:233, :244).  Clone c of word w shares that word's couplings and draws its initial spins and
+ *                  Metropolis uniforms as the virtual word w + c*2^20 (Q25).  The handle then has
+ *                  64*n_words*n_clones lanes, clone-major: lane = c*64*n_words + 64*w + b; every per-lane output and
+ *                  sg_get_spins / sg_set_spins (n_words*n_clones words per site) follow that order.
+ *   aligned_start  1: every spin starts at +1 ("the initial configuration has all the spins aligned", PAPER.md:231;
+ *                  DESIGN.md Q26) instead of the random start.
+ */
+typedef struct sg_options {
+    uint32_t word0;
+    uint32_t n_clones;        /* 0 is read as 1 */
+    uint32_t aligned_start;
+    uint32_t reserved;        /* must be 0 */
+} sg_options;
+sg_sim *sg_create_opt(int model, uint64_t N, double c, double T, uint64_t seed, uint32_t n_words, const sg_options *opt);
+/* Number of lanes of the handle: 64 * n_words * n_clones. */
+uint64_t sg_num_lanes(const sg_sim *h);
+
 /* Release everything the handle owns (synchronises the stream first).  NULL is allowed. */
 void sg_destroy(sg_sim *h);
 
@@ -73,7 +97,7 @@ int sg_snapshot(sg_sim *h, uint32_t slot);
 /*
  * sg_correlation -- out_counts[l] = D_l = #{ i : s_i(now) != s_i(slot) } for every lane l,
  * so that C(tw, tw+t) = 1 - 2*D_l/N.  Exact integers.
- *   out_counts  HOST, 64*n_words uint64.
+ *   out_counts  HOST, sg_num_lanes() = 64*n_words(*n_clones) uint64.
  * Synchronises the stream.  SG_ESLOT if the slot was never written.
  */
 int sg_correlation(sg_sim *h, uint32_t slot, uint64_t *out_counts);
@@ -82,10 +106,27 @@ int sg_correlation(sg_sim *h, uint32_t slot, uint64_t *out_counts);
  * sg_energy -- per-lane energy of the current configuration, exact integers.
  *   VB: out[l] = E_l  = -sum_{(ij) in E} J_ij s_i s_j
  *   SK: out[l] = E'_l = -sum_{i<j} J'_ij s_i s_j with J' = +-1; energy = E'_l / sqrt(N)
- *   out  HOST, 64*n_words int64.
+ *   out  HOST, sg_num_lanes() int64.
  * Synchronises the stream.
  */
 int sg_energy(sg_sim *h, int64_t *out);
+
+/*
+ * Windowed measurement (PAPER.md:95 "averaged over the time window", :270 minor-third intervals of tw + t; :233 tritone
+ * lumps for SK): the paper averages C(tw, tw+t) over every sweep of a logarithmic time window, for several stored tw at
+ * once.  These calls keep that bookkeeping on the device: bins of exact per-lane sums of D, nothing crosses PCIe and
+ * nothing synchronises until the fetch.
+ *   sg_corr_configure   allocate nbins accumulators (sg_num_lanes() uint64 each) and zero them, and their hit counts.
+ *   sg_corr_accumulate  for k < n: acc[bins[k]][l] += D_l(now, slot slots[k]) and hits[bins[k]] += 1.  Asynchronous.  The
+ *                       current configuration is read once per group of three slots (8 + 8S bytes per site-word instead
+ *                       of 16 S).  slots, bins: HOST, n uint32; the bins of one call must be distinct; SG_ESLOT if a slot
+ *                       was never written.
+ *   sg_corr_fetch       out[b*lanes + l] = acc[bin0 + b][l] (HOST, nbins*lanes uint64), n_out[b] = hits (HOST, may be
+ *                       NULL).  Synchronises the stream.  The caller's window average is C = 1 - 2*acc / (hits * N).
+ */
+int sg_corr_configure(sg_sim *h, uint32_t nbins);
+int sg_corr_accumulate(sg_sim *h, uint32_t n, const uint32_t *slots, const uint32_t *bins);
+int sg_corr_fetch(sg_sim *h, uint32_t bin0, uint32_t nbins, uint64_t *out, uint64_t *n_out);
 
 /* Message of the last failure on this thread ("" if none). */
 const char *sg_last_error(void);

@@ -41,11 +41,14 @@ def lib() -> C.CDLL:
         L.or_philox.restype = None
         L.or_create.argtypes = [C.c_int, u64, dbl, dbl, u64, u32]
         L.or_create.restype = vp
+        L.or_create_opt.argtypes = [C.c_int, u64, dbl, dbl, u64, u32, u32, u32, C.c_int]
+        L.or_create_opt.restype = vp
         L.or_create_explicit.argtypes = [u64, u64, vp, vp, vp, vp, dbl, u64, u32]
         L.or_create_explicit.restype = vp
         L.or_destroy.argtypes = [vp]
         L.or_destroy.restype = None
         L.or_sweep.argtypes = [vp, u64]
+        L.or_sk_update_range.argtypes = [vp, u64, u64]
         L.or_snapshot.argtypes = [vp, u32]
         L.or_correlation.argtypes = [vp, u32, vp]
         L.or_energy.argtypes = [vp, vp]
@@ -82,13 +85,16 @@ def philox(c0, c1, c2, c3, k0, k1) -> np.ndarray:
 class Oracle:
     """Thin handle around or_sim*.  Mirrors the sg_* call names."""
 
-    def __init__(self, model: int, N: int, c: float, T: float, seed: int, n_words: int, _handle=None):
+    def __init__(self, model: int, N: int, c: float, T: float, seed: int, n_words: int, _handle=None,
+                 word0: int = 0, n_clones: int = 1, aligned_start: bool = False):
         self._L = lib()
         self.model, self.N, self.c, self.T, self.seed, self.W = model, int(N), c, T, seed, int(n_words)
-        self._h = _handle if _handle is not None else self._L.or_create(model, N, c, T, seed, n_words)
+        self.word0, self.n_clones, self.aligned_start = int(word0), int(n_clones), bool(aligned_start)
+        self._h = _handle if _handle is not None else self._L.or_create_opt(model, N, c, T, seed, n_words, self.word0,
+                                                                           self.n_clones, int(self.aligned_start))
         if not self._h:
             raise ValueError("or_create rejected the arguments")
-        self.lanes = 64 * self.W
+        self.lanes = 64 * self.W * self.n_clones
 
     @classmethod
     def explicit(cls, N, edges, kappa, sigma, T, seed=0, n_words=1):
@@ -119,6 +125,10 @@ class Oracle:
     # --- the five calls
     def sweep(self, n: int = 1):
         rc = self._L.or_sweep(self._h, n)
+        assert rc == 0
+
+    def sk_update_range(self, i0: int, i1: int):
+        rc = self._L.or_sk_update_range(self._h, i0, i1)
         assert rc == 0
 
     def snapshot(self, slot: int):
@@ -157,14 +167,14 @@ class Oracle:
         return self._L.or_max_degree(self._h)
 
     def spins(self, slot: int = -1) -> np.ndarray:
-        out = np.zeros((self.N, self.W), dtype=np.uint64)
+        out = np.zeros((self.N, self.W * self.n_clones), dtype=np.uint64)
         rc = self._L.or_get_spins(self._h, slot, _p(out))
         if rc != 0:
             raise RuntimeError(f"or_get_spins -> {rc}")
         return out
 
     def set_spins(self, words: np.ndarray):
-        words = np.ascontiguousarray(np.asarray(words, dtype=np.uint64).reshape(self.N, self.W))
+        words = np.ascontiguousarray(np.asarray(words, dtype=np.uint64).reshape(self.N, self.W * self.n_clones))
         self._L.or_set_spins(self._h, _p(words))
 
     def set_sweep_count(self, t: int):

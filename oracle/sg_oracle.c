@@ -33,8 +33,20 @@
  * exact enumeration / Boltzmann (P3), full transition matrix and detailed
  * balance (P4), C(tw,tw)=1 (P5), energy bookkeeping (P6), T=0 (P7), T=inf
  * (P8), forced cases (P9), generator statistics (P10), paramagnet energy (P12),
- * SK small-N (P13).  Unpinned by the paper: the numerical values of
- * C(tw,tw+t) themselves (no number is printed).
+ * SK small-N (P13), word offset / clones / aligned start (P15).  Unpinned by the
+ * paper: the numerical values of C(tw,tw+t) themselves (no number is printed;
+ * see DESIGN.md).
+ *
+ * Options (or_create_opt; readings Q24-Q26), all neutral at their defaults:
+ *   word0    the handle simulates words word0 .. word0+W-1 of the instance: every
+ *            Philox counter that takes a word index takes word0 + w (Q16: words
+ *            are independent given the graph, so a W-word run is W one-word runs)
+ *   clones   SK: "two clones (i.e. replicas with the same
+ *            couplings)": clone c shares the coupling words of word w and draws
+ *            its initial spins and its Metropolis uniforms as the virtual word
+ *            w + c * 2^20 (Q25)
+ *   aligned  PAPER.md:231: "the initial configuration has all the spins
+ *            aligned": every spin +1 at t = 0 (Q26)
  */
 #include <stdint.h>
 #include <stdlib.h>
@@ -71,7 +83,18 @@ typedef struct or_sim {
     int8_t   *slot[OR_MAX_SLOTS];
     int64_t  *dE;       /* per-lane accumulated energy change (VB: units of J; SK: numerator) */
     uint64_t *nflip;    /* per-lane number of accepted flips in the last sweep */
+    uint32_t  word0;    /* first word of the instance this handle simulates */
+    uint32_t  clones;   /* replicas sharing the couplings: lane = c*64*W + 64*w + b */
+    int       aligned;  /* all spins +1 initially */
 } or_sim;
+
+#define OR_CLONE_STRIDE (1u << 20)   /* virtual word of clone c of word w: w + c * 2^20 */
+
+/* word index that the Philox counters of spins and uniforms use for lane group (clone c, word w) */
+static uint32_t virtual_word(const or_sim *h, uint32_t c, uint32_t w)
+{
+    return h->word0 + w + c * OR_CLONE_STRIDE;
+}
 
 /* ------------------------------------------------------------------ O1 */
 /* Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11): 10 rounds of
@@ -120,6 +143,8 @@ static int jbit(const uint64_t *kappa_words, uint64_t lane)
     uint64_t word = kappa_words[lane >> 6];
     return ((word >> (lane & 63)) & 1u) ? -1 : +1;
 }
+/* the clones of a word share its couplings: coupling lane of lane l = l mod 64*W */
+#define CL(h, lane) ((lane) % (64ull * (h)->W))
 
 static uint64_t sk_pair(uint64_t N, uint64_t i, uint64_t j)
 {
@@ -176,7 +201,8 @@ static int build_csr_colour_thr(or_sim *h)
 
 static int alloc_state(or_sim *h)
 {
-    h->L = 64ull * h->W;
+    if (h->clones == 0) h->clones = 1;
+    h->L = 64ull * h->W * h->clones;
     h->s = (int8_t *)malloc(h->N * h->L);
     h->dE = (int64_t *)calloc(h->L, sizeof(int64_t));
     h->nflip = (uint64_t *)calloc(h->L, sizeof(uint64_t));
@@ -196,23 +222,28 @@ void or_destroy(or_sim *h)
 static void draw_initial_spins(or_sim *h)
 {
     for (uint64_t i = 0; i < h->N; ++i)
-        for (uint32_t w = 0; w < h->W; ++w) {
-            uint32_t x[4];
-            P(h, (uint32_t)i, w, 0, 1, x);
-            uint64_t sigma = (uint64_t)x[0] | ((uint64_t)x[1] << 32);
-            for (int b = 0; b < 64; ++b)
-                h->s[i * h->L + 64ull * w + b] = ((sigma >> b) & 1u) ? -1 : +1;
-        }
+        for (uint32_t c = 0; c < h->clones; ++c)
+            for (uint32_t w = 0; w < h->W; ++w) {
+                uint32_t x[4];
+                P(h, (uint32_t)i, virtual_word(h, c, w), 0, 1, x);
+                uint64_t sigma = (uint64_t)x[0] | ((uint64_t)x[1] << 32);
+                for (int b = 0; b < 64; ++b)
+                    h->s[i * h->L + 64ull * (c * h->W + w) + b] = (!h->aligned && ((sigma >> b) & 1u)) ? -1 : +1;
+            }
 }
 
-or_sim *or_create(int model, uint64_t N, double c, double T, uint64_t seed, uint32_t n_words)
+or_sim *or_create_opt(int model, uint64_t N, double c, double T, uint64_t seed, uint32_t n_words,
+                      uint32_t word0, uint32_t clones, int aligned)
 {
     if (N < 2 || N >= (1ull << 32) || n_words == 0) return NULL;
     if (model != OR_VB && model != OR_SK && model != OR_RRBG) return NULL;
     if (model == OR_RRBG && (N < 8 || (N & 1))) return NULL;   /* two halves of N/2 >= 4 vertices */
     if (!(T >= 0.0)) return NULL;
+    if (clones < 1 || clones > 2 || (clones > 1 && model != OR_SK)) return NULL;
+    if ((uint64_t)word0 + n_words > OR_CLONE_STRIDE) return NULL;
     or_sim *h = (or_sim *)calloc(1, sizeof(or_sim));
     h->model = model; h->N = N; h->W = n_words; h->T = T; h->seed = seed; h->sweep = 0;
+    h->word0 = word0; h->clones = clones; h->aligned = aligned;
     if (alloc_state(h)) { or_destroy(h); return NULL; }
 
     if (model == OR_RRBG) {
@@ -258,7 +289,7 @@ or_sim *or_create(int model, uint64_t N, double c, double T, uint64_t seed, uint
         for (uint64_t f = 0; f < M; ++f)
             for (uint32_t w = 0; w < h->W; ++w) {
                 uint32_t x[4];
-                P(h, (uint32_t)f, w, 0, 2, x);
+                P(h, (uint32_t)f, h->word0 + w, 0, 2, x);
                 h->kappa[f * h->W + w] = (uint64_t)x[0] | ((uint64_t)x[1] << 32);
             }
     } else if (model == OR_VB) {
@@ -300,7 +331,7 @@ or_sim *or_create(int model, uint64_t N, double c, double T, uint64_t seed, uint
         for (uint64_t f = 0; f < M; ++f)
             for (uint32_t w = 0; w < h->W; ++w) {
                 uint32_t x[4];
-                P(h, (uint32_t)f, w, 0, 2, x);
+                P(h, (uint32_t)f, h->word0 + w, 0, 2, x);
                 h->kappa[f * h->W + w] = (uint64_t)x[0] | ((uint64_t)x[1] << 32);
             }
     } else {
@@ -312,7 +343,7 @@ or_sim *or_create(int model, uint64_t N, double c, double T, uint64_t seed, uint
             for (uint64_t j = i + 1; j < N; ++j)
                 for (uint32_t w = 0; w < h->W; ++w) {
                     uint32_t x[4];
-                    P(h, (uint32_t)j, w, i, 2, x);
+                    P(h, (uint32_t)j, h->word0 + w, i, 2, x);
                     h->kappa[sk_pair(N, i, j) * h->W + w] = (uint64_t)x[0] | ((uint64_t)x[1] << 32);
                 }
         h->nthr = N;
@@ -322,6 +353,11 @@ or_sim *or_create(int model, uint64_t N, double c, double T, uint64_t seed, uint
     }
     draw_initial_spins(h);
     return h;
+}
+
+or_sim *or_create(int model, uint64_t N, double c, double T, uint64_t seed, uint32_t n_words)
+{
+    return or_create_opt(model, N, c, T, seed, n_words, 0, 1, 0);
 }
 
 /* Explicit VB instance for the pins: edges (u[e],v[e]), coupling words
@@ -356,23 +392,25 @@ or_sim *or_create_explicit(uint64_t N, uint64_t M, const uint32_t *u, const uint
  * P(i, w>>2, t, tag 0); shared by the 64 lanes of the word (Q6). */
 static uint32_t uniform_for(const or_sim *h, uint64_t i, uint32_t w, uint64_t t)
 {
+    /* w counts lane groups of 64: w = c*W + (word inside the handle) */
+    uint32_t vw = virtual_word(h, w / h->W, w % h->W);
     uint32_t x[4];
-    P(h, (uint32_t)i, w >> 2, t, 0, x);
-    return x[w & 3];
+    P(h, (uint32_t)i, vw >> 2, t, 0, x);
+    return x[vw & 3];
 }
 
 static void vb_update_site(or_sim *h, uint64_t i, uint64_t t)
 {
     uint64_t L = h->L;
     int64_t d = (int64_t)(h->row_ptr[i + 1] - h->row_ptr[i]);
-    for (uint32_t w = 0; w < h->W; ++w) {
+    for (uint32_t w = 0; w < h->W * h->clones; ++w) {
         uint32_t r = uniform_for(h, i, w, t);
         for (int b = 0; b < 64; ++b) {
             uint64_t lane = 64ull * w + b;
             int64_t u = 0;   /* unsatisfied bonds: s_i s_j J = -1 */
             for (uint64_t a = h->row_ptr[i]; a < h->row_ptr[i + 1]; ++a) {
                 uint64_t j = h->adj[a];
-                int J = jbit(&h->kappa[h->adj_e[a] * h->W], lane);
+                int J = jbit(&h->kappa[h->adj_e[a] * h->W], CL(h, lane));
                 if ((int)h->s[i * L + lane] * (int)h->s[j * L + lane] * J == -1) u++;
             }
             int64_t kk = d - 2 * u;          /* Delta E = 2*kk */
@@ -388,7 +426,7 @@ static void vb_update_site(or_sim *h, uint64_t i, uint64_t t)
 static void sk_update_site(or_sim *h, uint64_t i, uint64_t t)
 {
     uint64_t L = h->L, N = h->N;
-    for (uint32_t w = 0; w < h->W; ++w) {
+    for (uint32_t w = 0; w < h->W * h->clones; ++w) {
         uint32_t r = uniform_for(h, i, w, t);
         for (int b = 0; b < 64; ++b) {
             uint64_t lane = 64ull * w + b;
@@ -396,7 +434,7 @@ static void sk_update_site(or_sim *h, uint64_t i, uint64_t t)
             for (uint64_t j = 0; j < N; ++j) {
                 if (j == i) continue;
                 uint64_t p = (i < j) ? sk_pair(N, i, j) : sk_pair(N, j, i);
-                H += (int64_t)jbit(&h->kappa[p * h->W], lane) * (int64_t)h->s[j * L + lane];
+                H += (int64_t)jbit(&h->kappa[p * h->W], CL(h, lane)) * (int64_t)h->s[j * L + lane];
             }
             int64_t m = (int64_t)h->s[i * L + lane] * H;   /* Delta E = 2 m / sqrt N */
             if (m <= 0 || (uint64_t)r < h->thr[m]) {
@@ -423,6 +461,17 @@ int or_sweep(or_sim *h, uint64_t n)
         }
         h->sweep = t + 1;
     }
+    return 0;
+}
+
+/* SK only: the updates of sites i0 .. i1-1 of the sweep with the current index, in order, on the current
+ * configuration; the sweep counter does not move.  A sweep is the composition of its N site updates ("N
+ * single spin updates, performed in a fixed order"), so tests can check a window of a very large instance: sites
+ * below i0 already carry their new values, the others their old ones. */
+int or_sk_update_range(or_sim *h, uint64_t i0, uint64_t i1)
+{
+    if (!h || h->model != OR_SK || i0 > i1 || i1 > h->N) return -1;
+    for (uint64_t i = i0; i < i1; ++i) sk_update_site(h, i, h->sweep);
     return 0;
 }
 
@@ -458,13 +507,13 @@ int or_energy(or_sim *h, int64_t *out)
         int64_t E = 0;
         if (h->model == OR_VB) {
             for (uint64_t e = 0; e < h->M; ++e)
-                E -= (int64_t)jbit(&h->kappa[e * h->W], lane)
+                E -= (int64_t)jbit(&h->kappa[e * h->W], CL(h, lane))
                    * (int64_t)h->s[(uint64_t)h->eu[e] * L + lane]
                    * (int64_t)h->s[(uint64_t)h->ev[e] * L + lane];
         } else {
             for (uint64_t i = 0; i < h->N; ++i)
                 for (uint64_t j = i + 1; j < h->N; ++j)
-                    E -= (int64_t)jbit(&h->kappa[sk_pair(h->N, i, j) * h->W], lane)
+                    E -= (int64_t)jbit(&h->kappa[sk_pair(h->N, i, j) * h->W], CL(h, lane))
                        * (int64_t)h->s[i * L + lane] * (int64_t)h->s[j * L + lane];
         }
         out[lane] = E;
@@ -479,7 +528,7 @@ uint32_t or_num_colours(const or_sim *h) { return h->K; }
 uint32_t or_max_degree(const or_sim *h) { return h->dmax; }
 
 /* packed spin words in original site order, word-minor: out[i*W+w], bit 1 <=> s=-1.
- * slot = -1: current configuration. */
+ * slot = -1: current configuration.  With clones: out[i*(W*clones) + c*W + w]. */
 int or_get_spins(const or_sim *h, int32_t slot, uint64_t *out)
 {
     const int8_t *src = h->s;
@@ -487,12 +536,13 @@ int or_get_spins(const or_sim *h, int32_t slot, uint64_t *out)
         if (slot >= OR_MAX_SLOTS || !h->slot[slot]) return -4;
         src = h->slot[slot];
     }
+    const uint64_t G = h->L / 64;    /* lane groups per site: W * clones, clone-major */
     for (uint64_t i = 0; i < h->N; ++i)
-        for (uint32_t w = 0; w < h->W; ++w) {
+        for (uint64_t w = 0; w < G; ++w) {
             uint64_t word = 0;
             for (int b = 0; b < 64; ++b)
                 if (src[i * h->L + 64ull * w + b] < 0) word |= (1ull << b);
-            out[i * h->W + w] = word;
+            out[i * G + w] = word;
         }
     return 0;
 }
@@ -502,7 +552,7 @@ int or_set_spins(or_sim *h, const uint64_t *in)
 {
     for (uint64_t i = 0; i < h->N; ++i)
         for (uint64_t lane = 0; lane < h->L; ++lane)
-            h->s[i * h->L + lane] = ((in[i * h->W + (lane >> 6)] >> (lane & 63)) & 1u) ? -1 : +1;
+            h->s[i * h->L + lane] = ((in[i * (h->L / 64) + (lane >> 6)] >> (lane & 63)) & 1u) ? -1 : +1;
     return 0;
 }
 

@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     load_library,
     sg_correlation,
     sg_create,
+    sg_create_opt,
     sg_destroy,
     sg_energy,
     sg_snapshot,

@@ -20,11 +20,16 @@ LIB_PATH = os.environ.get("SG_LIBSG_PATH") or os.path.join(_HERE, "libsg.so")   
 _u64, _u32, _i32, _dbl, _vp = C.c_uint64, C.c_uint32, C.c_int32, C.c_double, C.c_void_p
 SYMBOLS = {
     "sg_create": (_vp, [C.c_int, _u64, _dbl, _dbl, _u64, _u32]),
+    "sg_create_opt": (_vp, [C.c_int, _u64, _dbl, _dbl, _u64, _u32, _vp]),
+    "sg_num_lanes": (_u64, [_vp]),
     "sg_destroy": (None, [_vp]),
     "sg_sweep": (C.c_int, [_vp, _u64]),
     "sg_snapshot": (C.c_int, [_vp, _u32]),
     "sg_correlation": (C.c_int, [_vp, _u32, _vp]),
     "sg_energy": (C.c_int, [_vp, _vp]),
+    "sg_corr_configure": (C.c_int, [_vp, _u32]),
+    "sg_corr_accumulate": (C.c_int, [_vp, _u32, _vp, _vp]),
+    "sg_corr_fetch": (C.c_int, [_vp, _u32, _u32, _vp, _vp]),
     "sg_last_error": (C.c_char_p, []),
     "sg_sweep_count": (_u64, [_vp]),
     "sg_num_edges": (_u64, [_vp]),
@@ -99,6 +104,23 @@ def sg_create(model: int, N: int, c: float, T: float, seed: int, n_words: int) -
     return h
 
 
+class sg_options(C.Structure):
+    _fields_ = [("word0", _u32), ("n_clones", _u32), ("aligned_start", _u32), ("reserved", _u32)]
+
+
+def sg_create_opt(model: int, N: int, c: float, T: float, seed: int, n_words: int, word0: int = 0, n_clones: int = 1,
+                  aligned_start: bool = False) -> int:
+    import torch
+
+    if torch.cuda.is_available():
+        torch.cuda.init()
+    opt = sg_options(int(word0), int(n_clones), 1 if aligned_start else 0, 0)
+    h = load_library().sg_create_opt(int(model), int(N), float(c), float(T), int(seed), int(n_words), C.byref(opt))
+    if not h:
+        raise SGError(SG_EINVAL, _err())
+    return h
+
+
 def sg_destroy(h: int) -> None:
     load_library().sg_destroy(h)
 
@@ -131,11 +153,18 @@ def kernel_launches() -> int:
 class Sim:
     """Owns one sg_sim*.  Methods mirror the C calls one to one."""
 
-    def __init__(self, model: int, N: int, c: float, T: float, seed: int, n_words: int):
+    def __init__(self, model: int, N: int, c: float, T: float, seed: int, n_words: int, word0: int = 0, n_clones: int = 1,
+                 aligned_start: bool = False):
         self._L = load_library()
         self.model, self.N, self.c, self.T, self.seed, self.W = model, int(N), float(c), float(T), int(seed), int(n_words)
-        self.lanes = 64 * self.W
-        self._h = sg_create(model, N, c, T, seed, n_words)
+        self.word0, self.n_clones, self.aligned_start = int(word0), int(n_clones), bool(aligned_start)
+        self.groups = self.W * self.n_clones          # 64-lane groups per site
+        self.lanes = 64 * self.groups
+        if word0 == 0 and n_clones == 1 and not aligned_start:
+            self._h = sg_create(model, N, c, T, seed, n_words)
+        else:
+            self._h = sg_create_opt(model, N, c, T, seed, n_words, word0, n_clones, aligned_start)
+        assert self._L.sg_num_lanes(self._h) == self.lanes
 
     def close(self):
         if getattr(self, "_h", None):
@@ -168,6 +197,21 @@ class Sim:
         out = np.zeros(self.lanes, dtype=np.int64) if out is None else out
         return sg_energy(self._h, out)
 
+    def corr_configure(self, nbins: int):
+        _check(self._L.sg_corr_configure(self._h, int(nbins)))
+
+    def corr_accumulate(self, slots, bins):
+        slots = np.ascontiguousarray(np.asarray(slots, dtype=np.uint32))
+        bins = np.ascontiguousarray(np.asarray(bins, dtype=np.uint32))
+        assert slots.shape == bins.shape
+        _check(self._L.sg_corr_accumulate(self._h, slots.size, _ptr(slots), _ptr(bins)))
+
+    def corr_fetch(self, bin0: int, nbins: int):
+        out = np.zeros((nbins, self.lanes), dtype=np.uint64)
+        hits = np.zeros(nbins, dtype=np.uint64)
+        _check(self._L.sg_corr_fetch(self._h, int(bin0), int(nbins), _ptr(out), _ptr(hits)))
+        return out, hits
+
     @property
     def sweep_count(self) -> int:
         return self._L.sg_sweep_count(self._h)
@@ -186,13 +230,13 @@ class Sim:
 
     def spins(self, slot: int = -1, out: np.ndarray | None = None) -> np.ndarray:
         if out is None:
-            out = np.zeros((self.N, self.W), dtype=np.uint64)
-        assert out.dtype == np.uint64 and out.flags.c_contiguous and out.size == self.N * self.W
+            out = np.zeros((self.N, self.groups), dtype=np.uint64)
+        assert out.dtype == np.uint64 and out.flags.c_contiguous and out.size == self.N * self.groups
         _check(self._L.sg_get_spins(self._h, slot, _ptr(out)))
         return out
 
     def set_spins(self, words: np.ndarray):
-        words = np.ascontiguousarray(np.asarray(words, dtype=np.uint64).reshape(self.N, self.W))
+        words = np.ascontiguousarray(np.asarray(words, dtype=np.uint64).reshape(self.N, self.groups))
         _check(self._L.sg_set_spins(self._h, _ptr(words)))
 
     def set_sweep_count(self, t: int):

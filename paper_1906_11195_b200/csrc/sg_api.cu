@@ -68,15 +68,15 @@ int create_vb(sg_sim *h)
         for (uint64_t q = 0; q < N; ++q) {
             const uint64_t p = g.bfs_pos[q], par = g.tpar[p];
             if (par == SG_NONE) continue;
-            for (uint32_t w = 0; w < W; ++w) eps[p * W + w] = eps[par * W + w] ^ host_coupling_word(g.teid[p], w, h->key);
+            for (uint32_t w = 0; w < W; ++w) eps[p * W + w] = eps[par * W + w] ^ host_coupling_word(g.teid[p], h->word0 + w, h->key);
         }
     if (!upload(h->vb.col, g.col, st) || !upload(h->vb.orig, g.orig, st) || !upload(h->vb.orig_s, g.orig_s, st) ||
         !upload(h->vb.rp_s, g.rp_s, st) || !upload(h->vb.hdr, g.hdr, st) ||
         !upload(jeid_dev, g.jeid, st) || !upload(h->vb.eps, eps, st))
         return SG_ECUDA;
-    int rc = sgk_init_vb_couplings(h->vb, jeid_dev, h->W, h->key, st);
+    int rc = sgk_init_vb_couplings(h->vb, jeid_dev, h->W, h->word0, h->key, st);
     if (rc) return rc;
-    rc = sgk_init_spins(h->vb.spin, h->vb.orig, h->vb.eps, N, h->W, h->key, st);
+    rc = sgk_init_spins(h->vb.spin, h->vb.orig, h->vb.eps, N, h->W, h->word0, h->aligned, h->key, st);
     if (rc) return rc;
     if (!cuda_ok(cudaStreamSynchronize(st), "sg_create")) return SG_ECUDA;
     // the entry->edge table is only needed to draw the couplings; the large host copies are not needed any more
@@ -93,7 +93,20 @@ int create_vb(sg_sim *h)
 
 extern "C" sg_sim *sg_create(int model, uint64_t N, double c, double T, uint64_t seed, uint32_t n_words)
 {
+    return sg_create_opt(model, N, c, T, seed, n_words, nullptr);
+}
+
+extern "C" uint64_t sg_num_lanes(const sg_sim *h) { return h ? h->lanes : 0; }
+
+extern "C" sg_sim *sg_create_opt(int model, uint64_t N, double c, double T, uint64_t seed, uint32_t n_words, const sg_options *opt)
+{
     g_err.clear();
+    sg_options o{0, 1, 0, 0};
+    if (opt) o = *opt;
+    if (o.n_clones == 0) o.n_clones = 1;
+    if (o.reserved != 0 || o.aligned_start > 1) { sg_set_error("sg_create_opt: bad options"); return nullptr; }
+    if (o.n_clones > 2 || (o.n_clones == 2 && model != SG_MODEL_SK)) { sg_set_error("sg_create_opt: n_clones must be 1, or 2 for the SK model"); return nullptr; }
+    if (o.word0 % 4 != 0 || (uint64_t)o.word0 + n_words > (1u << 20)) { sg_set_error("sg_create_opt: word0 must be a multiple of 4 and word0 + n_words <= 2^20"); return nullptr; }
     if (model != SG_MODEL_VB && model != SG_MODEL_SK && model != SG_MODEL_RRBG) { sg_set_error("sg_create: unknown model"); return nullptr; }
     if (N < 2 || N >= (1ull << 31) - 2) { sg_set_error("sg_create: N must satisfy 2 <= N < 2^31 - 2"); return nullptr; }
     if (n_words == 0 || n_words > 65535) { sg_set_error("sg_create: n_words must satisfy 1 <= n_words <= 65535"); return nullptr; }
@@ -107,12 +120,14 @@ extern "C" sg_sim *sg_create(int model, uint64_t N, double c, double T, uint64_t
     h->graph_model = model;
     if (model == SG_MODEL_RRBG) model = SG_MODEL_VB;
     h->model = model; h->N = N; h->W = n_words; h->c = c; h->T = T; h->seed = seed;
+    h->word0 = o.word0; h->clones = o.n_clones; h->aligned = o.aligned_start != 0;
+    h->lanes = 64ull * n_words * o.n_clones;
     h->key = SGSeed{(uint32_t)seed, (uint32_t)(seed >> 32)};
     int rc;
     try {
         rc = (model == SG_MODEL_VB) ? create_vb(h) : sg_sk_create_impl(h);
         if (rc == SG_OK) {
-            h->counts_dev = dev_alloc<uint64_t>(h, 64ull * n_words);
+            h->counts_dev = dev_alloc<uint64_t>(h, h->lanes);
             if (!h->counts_dev) rc = SG_ENOMEM;
         }
     } catch (const std::bad_alloc &) {
@@ -133,7 +148,7 @@ extern "C" int sg_sweep(sg_sim *h, uint64_t n)
     cudaStream_t st = sgx_stream();
     for (uint64_t it = 0; it < n; ++it) {
         for (uint32_t k = 0; k < h->g.K; ++k) {
-            const int rc = sgk_vb_sweep_class(h->vb, h->g.cls[k], h->g.N, h->vb_nJ, h->W, h->sweep, h->key, h->vb_reverse, st);
+            const int rc = sgk_vb_sweep_class(h->vb, h->g.cls[k], h->g.N, h->vb_nJ, h->W, h->word0, h->sweep, h->key, h->vb_reverse, st);
             h->vb_reverse = !h->vb_reverse;
             if (rc) return rc;
         }
@@ -164,7 +179,7 @@ extern "C" int sg_correlation(sg_sim *h, uint32_t slot, uint64_t *out_counts)
     if (slot >= SG_MAX_SLOTS) { sg_set_error("sg_correlation: slot out of range"); return SG_EINVAL; }
     if (!h->slot[slot]) { sg_set_error("sg_correlation: slot was never written"); return SG_ESLOT; }
     cudaStream_t st = sgx_stream();
-    const uint64_t lanes = 64ull * h->W;
+    const uint64_t lanes = h->lanes;
     if (!cuda_ok(cudaMemsetAsync(h->counts_dev, 0, lanes * 8, st), "sg_correlation")) return SG_ECUDA;
     if (h->model == SG_MODEL_SK) return sg_sk_correlation_impl(h, h->slot[slot], out_counts);
     // position order in both operands (the same permutation), so no relabelling is needed
@@ -176,12 +191,69 @@ extern "C" int sg_correlation(sg_sim *h, uint32_t slot, uint64_t *out_counts)
     return SG_OK;
 }
 
+// ---- windowed protocol: device-side accumulation of correlation counts ---------------------
+extern "C" int sg_corr_configure(sg_sim *h, uint32_t nbins)
+{
+    if (!h || nbins == 0 || nbins > (1u << 20)) { sg_set_error("sg_corr_configure: bad argument"); return SG_EINVAL; }
+    cudaStream_t st = sgx_stream();
+    if (nbins > h->corr_bins) {
+        // (the old block stays with the handle until sg_destroy; reconfiguring to a larger size is rare)
+        h->corr_acc = dev_alloc<uint64_t>(h, (uint64_t)nbins * h->lanes);
+        if (!h->corr_acc) { h->corr_bins = 0; return SG_ENOMEM; }
+        h->corr_bins = nbins;
+    }
+    h->corr_n.assign(h->corr_bins, 0);
+    if (!cuda_ok(cudaMemsetAsync(h->corr_acc, 0, (uint64_t)h->corr_bins * h->lanes * 8, st), "sg_corr_configure")) return SG_ECUDA;
+    return SG_OK;
+}
+
+extern "C" int sg_corr_accumulate(sg_sim *h, uint32_t n, const uint32_t *slots, const uint32_t *bins)
+{
+    if (!h || (n && (!slots || !bins))) { sg_set_error("sg_corr_accumulate: null argument"); return SG_EINVAL; }
+    if (!h->corr_acc) { sg_set_error("sg_corr_accumulate: call sg_corr_configure first"); return SG_EINVAL; }
+    for (uint32_t k = 0; k < n; ++k) {
+        if (slots[k] >= SG_MAX_SLOTS || bins[k] >= h->corr_bins) { sg_set_error("sg_corr_accumulate: slot or bin out of range"); return SG_EINVAL; }
+        if (!h->slot[slots[k]]) { sg_set_error("sg_corr_accumulate: slot was never written"); return SG_ESLOT; }
+        for (uint32_t q = 0; q < k; ++q)
+            if (bins[q] == bins[k]) { sg_set_error("sg_corr_accumulate: the bins of one call must be distinct"); return SG_EINVAL; }
+    }
+    cudaStream_t st = sgx_stream();
+    for (uint32_t k0 = 0; k0 < n; k0 += 3) {
+        const uint32_t m = std::min<uint32_t>(3, n - k0);
+        const uint64_t *b[3];
+        uint64_t *c[3];
+        for (uint32_t q = 0; q < m; ++q) { b[q] = h->slot[slots[k0 + q]]; c[q] = h->corr_acc + (uint64_t)bins[k0 + q] * h->lanes; }
+        int rc = SG_OK;
+        if (h->model == SG_MODEL_SK) {
+            for (uint32_t q = 0; q < m && rc == SG_OK; ++q) rc = sg_sk_corr_accumulate_impl(h, b[q], c[q]);
+        } else {
+            rc = sgk_xor_popcount_multi(current_config(h), b, m, h->g.N, h->W, c, st);
+        }
+        if (rc) return rc;
+    }
+    for (uint32_t k = 0; k < n; ++k) h->corr_n[bins[k]]++;
+    return SG_OK;
+}
+
+extern "C" int sg_corr_fetch(sg_sim *h, uint32_t bin0, uint32_t nbins, uint64_t *out, uint64_t *n_out)
+{
+    if (!h || !out) { sg_set_error("sg_corr_fetch: null argument"); return SG_EINVAL; }
+    if (!h->corr_acc || (uint64_t)bin0 + nbins > h->corr_bins) { sg_set_error("sg_corr_fetch: bins out of range"); return SG_EINVAL; }
+    cudaStream_t st = sgx_stream();
+    if (nbins && (!cuda_ok(cudaMemcpyAsync(out, h->corr_acc + (uint64_t)bin0 * h->lanes, (uint64_t)nbins * h->lanes * 8, cudaMemcpyDeviceToHost, st),
+                           "sg_corr_fetch") ||
+                  !cuda_ok(cudaStreamSynchronize(st), "sg_corr_fetch")))
+        return SG_ECUDA;
+    if (n_out) for (uint32_t b = 0; b < nbins; ++b) n_out[b] = h->corr_n[bin0 + b];
+    return SG_OK;
+}
+
 extern "C" int sg_energy(sg_sim *h, int64_t *out)
 {
     if (!h || !out) { sg_set_error("sg_energy: null argument"); return SG_EINVAL; }
     if (h->model == SG_MODEL_SK) return sg_sk_energy_impl(h, out);
     cudaStream_t st = sgx_stream();
-    const uint64_t lanes = 64ull * h->W;
+    const uint64_t lanes = h->lanes;
     if (!cuda_ok(cudaMemsetAsync(h->counts_dev, 0, lanes * 8, st), "sg_energy")) return SG_ECUDA;
     const int rc = sgk_vb_unsat(h->vb, h->g.N, h->vb_nJ, h->W, h->counts_dev, st);
     if (rc) return rc;
@@ -206,7 +278,7 @@ extern "C" uint32_t sg_max_degree(const sg_sim *h)
 
 static bool ensure_scratch(sg_sim *h)
 {
-    if (!h->scratch) h->scratch = dev_alloc<uint64_t>(h, h->N * h->W);   // original order, no padding
+    if (!h->scratch) h->scratch = dev_alloc<uint64_t>(h, h->N * h->W);   // original order
     return h->scratch != nullptr;
 }
 

@@ -23,6 +23,23 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
+// the same with the ten round keys precomputed (rk[2r] = k0 + r*0x9E3779B9, rk[2r+1] = k1 + r*0xBB67AE85): the key
+// schedule then costs no instruction (the keys are operands from the constant bank)
+__device__ __forceinline__ void philox4x32_10_keys(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const uint32_t (&rk)[20],
+                                                   uint32_t (&out)[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t ha = __umulhi(0xD2511F53u, c0), la = 0xD2511F53u * c0;
+        const uint32_t hb = __umulhi(0xCD9E8D57u, c2), lb = 0xCD9E8D57u * c2;
+        c0 = hb ^ c1 ^ rk[2 * r];
+        c2 = ha ^ c3 ^ rk[2 * r + 1];
+        c1 = lb;
+        c3 = la;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
 // G consecutive 64-bit words (G = 1, 2, 4): one site's words of one word group
 template <int G> struct Vec { uint64_t v[G]; };
 

@@ -96,15 +96,19 @@ struct VBDevice {
 
 struct SGSeed { uint32_t k0, k1; };
 
-int sgk_init_spins(uint64_t *spin, const uint32_t *orig, const uint64_t *eps, uint64_t N, uint32_t W, SGSeed key, cudaStream_t st);
+int sgk_init_spins(uint64_t *spin, const uint32_t *orig, const uint64_t *eps, uint64_t N, uint32_t W, uint32_t word0, bool aligned, SGSeed key,
+                   cudaStream_t st);
 // draws every coupling entry (O3) and applies the gauge; jeid: device, edge id per coupling entry
-int sgk_init_vb_couplings(const VBDevice &d, const uint32_t *jeid, uint32_t W, SGSeed key, cudaStream_t st);
+int sgk_init_vb_couplings(const VBDevice &d, const uint32_t *jeid, uint32_t W, uint32_t word0, SGSeed key, cudaStream_t st);
 // one colour class of one sweep; N, nJ = sizes of the whole instance (choose 32- or 64-bit index arithmetic);
 // reverse = walk the class from its last slice to its first (callers alternate it from launch to launch)
-int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint64_t N, uint64_t nJ, uint32_t W, uint64_t sweep, SGSeed key,
+int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint64_t N, uint64_t nJ, uint32_t W, uint32_t word0, uint64_t sweep, SGSeed key,
                        bool reverse, cudaStream_t st);
 // counts[64*W] (device, u64) += per-lane number of set bits of (a XOR b) over n_sites*W words
 int sgk_xor_popcount(const uint64_t *a, const uint64_t *b, uint64_t n_sites, uint32_t W, uint64_t *counts, cudaStream_t st);
+// the same against up to 3 stored configurations in one pass: counts[s][64*W] += D(a, b[s])
+int sgk_xor_popcount_multi(const uint64_t *a, const uint64_t *const *b, uint32_t n, uint64_t n_sites, uint32_t W, uint64_t *const *counts,
+                           cudaStream_t st);
 // counts[64*W] += per-lane sum over all sites of u_i (unsatisfied incident bonds): one launch over the whole instance
 int sgk_vb_unsat(const VBDevice &d, uint64_t N, uint64_t nJ, uint32_t W, uint64_t *counts, cudaStream_t st);
 int sgk_permute_words(const uint64_t *src, uint64_t *dst, const uint32_t *map, const uint64_t *eps, uint64_t N, uint32_t W, bool scatter,

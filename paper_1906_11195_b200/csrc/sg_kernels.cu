@@ -26,15 +26,16 @@ void sgk_count_launch() { g_launches.fetch_add(1); }
 // ------------------------------------------------------------------------------------ init
 // O4: sigma_p[w] = x0 | x1<<32 of P(orig[p], w, 0, tag 1), stored gauge-transformed (^ eps); N here = number of positions
 __global__ void __launch_bounds__(256) k_init_spins(uint64_t *__restrict__ spin, const uint32_t *__restrict__ orig,
-                                                    const uint64_t *__restrict__ eps, uint64_t n, uint32_t W, uint32_t k0, uint32_t k1)
+                                                    const uint64_t *__restrict__ eps, uint64_t n, uint32_t W, uint32_t word0, int aligned,
+                                                    uint32_t k0, uint32_t k1)
 {
     for (uint64_t q = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (uint64_t)gridDim.x * blockDim.x) {
         const uint64_t p = q / W;
         const uint32_t w = (uint32_t)(q % W);
         const uint32_t site = orig ? orig[p] : (uint32_t)p;
         if (site == SG_NONE) { spin[q] = 0; continue; }   // padding position
-        uint32_t x[4];
-        philox4x32_10(site, w, 0u, 1u << 24, k0, k1, x);
+        uint32_t x[4] = {0, 0, 0, 0};
+        if (!aligned) philox4x32_10(site, word0 + w, 0u, 1u << 24, k0, k1, x);      // aligned start: every spin +1 (bit 0)
         spin[q] = ((uint64_t)x[0] | ((uint64_t)x[1] << 32)) ^ (eps ? eps[q] : 0ull);
     }
 }
@@ -45,10 +46,11 @@ static unsigned grid_for(uint64_t n, unsigned per_block)
     return (unsigned)std::min<uint64_t>(std::max<uint64_t>(b, 1), 1u << 20);     // grid-stride beyond 2^20 blocks
 }
 
-int sgk_init_spins(uint64_t *spin, const uint32_t *orig, const uint64_t *eps, uint64_t N, uint32_t W, SGSeed key, cudaStream_t st)
+int sgk_init_spins(uint64_t *spin, const uint32_t *orig, const uint64_t *eps, uint64_t N, uint32_t W, uint32_t word0, bool aligned, SGSeed key,
+                   cudaStream_t st)
 {
     const uint64_t n = N * W;
-    k_init_spins<<<grid_for(n, 256), 256, 0, st>>>(spin, orig, eps, n, W, key.k0, key.k1);
+    k_init_spins<<<grid_for(n, 256), 256, 0, st>>>(spin, orig, eps, n, W, word0, aligned ? 1 : 0, key.k0, key.k1);
     SG_LAUNCH_CHECK();
     return SG_OK;
 }
@@ -111,6 +113,83 @@ int sgk_xor_popcount(const uint64_t *a, const uint64_t *b, uint64_t n_sites, uin
         dim3 grid((unsigned)std::max<uint64_t>(1, blocks / W), W);
         k_xor_popcount<false><<<grid, 256, 0, st>>>(a, b, n_sites, W, (unsigned long long *)counts);
     }
+    SG_LAUNCH_CHECK();
+    return SG_OK;
+}
+
+// The same against S stored configurations in one pass over the current one (the windowed protocol of PAPER.md:95,
+// :270 counts against every stored waiting time after every sweep): 8 + 8 S bytes per site-word instead of 16 S.
+// W a power of two <= 32; counts are added to S separate rows.
+template <int S>
+__global__ void __launch_bounds__(256)
+k_xor_popcount_multi(const uint64_t *__restrict__ a, const uint64_t *__restrict__ b0, const uint64_t *__restrict__ b1,
+                     const uint64_t *__restrict__ b2, uint64_t total, uint32_t W, unsigned long long *__restrict__ c0,
+                     unsigned long long *__restrict__ c1, unsigned long long *__restrict__ c2)
+{
+    constexpr int P = 6, PT = P + 5;
+    uint64_t acc[S][PT];
+#pragma unroll
+    for (int s = 0; s < S; ++s) vc_clear(acc[s]);
+    const uint64_t *b[3] = {b0, b1, b2};
+    unsigned long long *c[3] = {c0, c1, c2};
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint64_t warp = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const uint64_t nwarps = ((uint64_t)gridDim.x * blockDim.x) >> 5;
+    const uint64_t pol_stream = policy_evict_first();
+    const uint64_t nchunks = (total + 31) / 32;
+    uint32_t pending = 0;
+    constexpr int U = 2;
+    for (uint64_t ch = warp; ch < nchunks; ch += (uint64_t)U * nwarps) {
+        uint64_t x[U], y[S][U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const uint64_t q = (ch + (uint64_t)u * nwarps) * 32 + lane;
+            x[u] = 0;
+#pragma unroll
+            for (int s = 0; s < S; ++s) y[s][u] = 0;
+            if (q < total) {
+                x[u] = ld_plain_u64(a + q);
+#pragma unroll
+                for (int s = 0; s < S; ++s) y[s][u] = ld_stream_u64(b[s] + q, pol_stream);
+            }
+        }
+#pragma unroll
+        for (int s = 0; s < S; ++s)
+#pragma unroll
+            for (int u = 0; u < U; ++u) vc_add_bit<P, PT>(acc[s], x[u] ^ y[s][u]);
+        pending += U;
+        if (pending + U > (1u << P) - 1u) {
+#pragma unroll
+            for (int s = 0; s < S; ++s) { vc_warp_flush<PT>(acc[s], W, 0, c[s]); vc_clear(acc[s]); }
+            pending = 0;
+        }
+    }
+    if (pending) {
+#pragma unroll
+        for (int s = 0; s < S; ++s) vc_warp_flush<PT>(acc[s], W, 0, c[s]);
+    }
+}
+
+// counts[s][64*W] += D(a, b[s]) for s < n (n <= 3); falls back to one pass per slot when W is not a power of two <= 32
+int sgk_xor_popcount_multi(const uint64_t *a, const uint64_t *const *b, uint32_t n, uint64_t n_sites, uint32_t W, uint64_t *const *counts,
+                           cudaStream_t st)
+{
+    const bool contig = W <= 32 && (W & (W - 1)) == 0;
+    if (!contig || n == 1) {
+        for (uint32_t s = 0; s < n; ++s) {
+            const int rc = sgk_xor_popcount(a, b[s], n_sites, W, counts[s], st);
+            if (rc) return rc;
+        }
+        return SG_OK;
+    }
+    const uint64_t total = n_sites * W;
+    uint64_t blocks = (total + 32 * 8 * 16 - 1) / (32 * 8 * 16);
+    if (blocks > 148 * 4) blocks = 148 * 4;
+    if (blocks < 1) blocks = 1;
+    auto cc = [&](uint32_t s) { return (unsigned long long *)counts[s < n ? s : 0]; };
+    auto bb = [&](uint32_t s) { return b[s < n ? s : 0]; };
+    if (n == 2) k_xor_popcount_multi<2><<<(unsigned)blocks, 256, 0, st>>>(a, bb(0), bb(1), bb(1), total, W, cc(0), cc(1), cc(1));
+    else k_xor_popcount_multi<3><<<(unsigned)blocks, 256, 0, st>>>(a, bb(0), bb(1), bb(2), total, W, cc(0), cc(1), cc(2));
     SG_LAUNCH_CHECK();
     return SG_OK;
 }

@@ -12,6 +12,9 @@ struct sg_sim {
     int graph_model = SG_MODEL_VB;           // the graph ensemble: SG_MODEL_VB (Erdos-Renyi) or SG_MODEL_RRBG
     uint64_t N = 0, M = 0;
     uint32_t W = 0;
+    uint32_t word0 = 0, clones = 1;         // sg_options
+    bool aligned = false;
+    uint64_t lanes = 0;                      // 64 * W * clones
     double c = 0, T = 0;
     uint64_t seed = 0;
     uint64_t sweep = 0;
@@ -29,6 +32,9 @@ struct sg_sim {
     uint64_t *slot[SG_MAX_SLOTS] = {nullptr};
     uint64_t *counts_dev = nullptr;          // 64*W
     uint64_t *scratch = nullptr;             // one configuration, for getters
+    uint64_t *corr_acc = nullptr;            // windowed protocol: corr_bins x lanes accumulated counts
+    uint32_t corr_bins = 0;
+    std::vector<uint64_t> corr_n;            // accumulations per bin
     std::vector<void *> owned;               // every device allocation
 };
 
@@ -60,6 +66,7 @@ int sg_sk_create_impl(sg_sim *h);
 int sg_sk_sweep_impl(sg_sim *h, uint64_t n);
 int sg_sk_energy_impl(sg_sim *h, int64_t *out);
 int sg_sk_correlation_impl(sg_sim *h, const uint64_t *slot_dev, uint64_t *out);
+int sg_sk_corr_accumulate_impl(sg_sim *h, const uint64_t *slot_dev, uint64_t *acc_dev);
 int sg_sk_get_spins_impl(sg_sim *h, const uint64_t *src_dev, uint64_t *out);
 int sg_sk_set_spins_impl(sg_sim *h, const uint64_t *in);
 int sg_sk_get_couplings_impl(sg_sim *h, uint64_t *out);

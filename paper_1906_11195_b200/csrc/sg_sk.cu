@@ -8,6 +8,8 @@
 //   rows  [lane][i][NW32]  u32   bit j%32 of word j/32 = 1 <=> J'_ij = -1 (diagonal and padding bits 0)
 //   H     [lane][Npad]     int16 integer local field H_i = sum_{j != i} J'_ij s_j, |H| <= N-1 <= 32767
 //   sbits [lane][NW32]     u32   bit = 1 <=> s = -1   (the SK configuration; snapshots use the same layout)
+// Clones (sg_options): lanes c*64W .. (c+1)*64W-1 are clone c; a clone shares the coupling rows of
+// lane (l mod 64W) and draws spins and uniforms as the virtual word word0 + w + c*2^20 (Q25).
 // One CTA owns one lane for a whole sg_sweep(n) call: fields, spins and the sweep's uniforms live in
 // shared memory; sites are visited in order in batches of 32.  Warp 0 decides a batch speculatively
 // (all 32 sites against the current fields, first acceptance by ballot + ffs, repair the 31 other
@@ -35,6 +37,7 @@ void sgk_count_launch();
 namespace {
 
 constexpr int SK_THREADS = 256;
+constexpr uint32_t SK_CLONE_STRIDE = 1u << 20;
 
 __host__ __device__ inline uint32_t sk_nw32(uint64_t N) { return (uint32_t)((N + 31) / 32); }
 // padded row length of the transposed field array in shared memory: 2 * odd, so that the 32 lanes of
@@ -44,7 +47,7 @@ __host__ __device__ inline uint32_t sk_nw32p(uint32_t nw32) { uint32_t h = (nw32
 // O3 (SK): kappa_ij[w] = x0 | x1<<32 of P(c0 = j, c1 = w, sweep field = i, tag 2) for i < j.
 // One warp per (i, word wq of j's, w): lane = j % 32 draws its coupling word, 64 ballots transpose
 // the 32 x 64 bit block into one u32 per lane.
-__global__ void __launch_bounds__(256) k_sk_init_rows(uint32_t *__restrict__ rows, uint64_t N, uint32_t NW32, uint32_t W,
+__global__ void __launch_bounds__(256) k_sk_init_rows(uint32_t *__restrict__ rows, uint64_t N, uint32_t NW32, uint32_t W, uint32_t word0,
                                                       uint32_t k0, uint32_t k1)
 {
     const uint64_t warp = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -59,7 +62,7 @@ __global__ void __launch_bounds__(256) k_sk_init_rows(uint32_t *__restrict__ row
     if (j < N && j != i) {
         const uint32_t lo = (uint32_t)(i < j ? i : j), hi = (uint32_t)(i < j ? j : i);
         uint32_t x[4];
-        philox4x32_10(hi, w, lo, 2u << 24, k0, k1, x);
+        philox4x32_10(hi, word0 + w, lo, 2u << 24, k0, k1, x);
         kappa = (uint64_t)x[0] | ((uint64_t)x[1] << 32);
     }
     uint32_t mine0 = 0, mine1 = 0;
@@ -76,12 +79,12 @@ __global__ void __launch_bounds__(256) k_sk_init_rows(uint32_t *__restrict__ row
 
 // H_i = sum_{j != i} J'_ij s_j = (N - 1) - 2 * #{ j != i : kappa_ij xor sigma_j = 1 }
 __global__ void __launch_bounds__(256) k_sk_init_fields(const uint32_t *__restrict__ rows, const uint32_t *__restrict__ sbits,
-                                                        int16_t *__restrict__ H, uint64_t N, uint32_t NW32)
+                                                        int16_t *__restrict__ H, uint64_t N, uint32_t NW32, uint32_t lanes_w)
 {
     const uint64_t lane_g = blockIdx.y;
     const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
-    const uint32_t *row = rows + (lane_g * N + i) * NW32;
+    const uint32_t *row = rows + ((lane_g % lanes_w) * N + i) * NW32;
     const uint32_t *sp = sbits + lane_g * NW32;
     uint32_t neg = 0;
     for (uint32_t wq = 0; wq < NW32; ++wq) {
@@ -93,20 +96,20 @@ __global__ void __launch_bounds__(256) k_sk_init_fields(const uint32_t *__restri
     H[lane_g * (32ull * NW32) + i] = (int16_t)((int)(N - 1) - 2 * (int)neg);
 }
 
-// O4 for the lane-major layout: bit (64w+b) of site i = bit b of x0|x1<<32 of P(i, w, 0, tag 1).
-// One warp per (32 sites, w): lane = site, 64 ballots transpose.
-__global__ void __launch_bounds__(256) k_sk_init_spins(uint32_t *__restrict__ sbits, uint64_t N, uint32_t NW32, uint32_t W,
-                                                       uint32_t k0, uint32_t k1)
+// O4 for the lane-major layout: bit (64w+b) of site i of clone c = bit b of x0|x1<<32 of P(i, word0 + w + c*2^20, 0, tag 1);
+// aligned start: every bit 0.  One warp per (32 sites, w, c): lane = site, 64 ballots transpose.
+__global__ void __launch_bounds__(256) k_sk_init_spins(uint32_t *__restrict__ sbits, uint64_t N, uint32_t NW32, uint32_t W, uint32_t clones,
+                                                       uint32_t word0, int aligned, uint32_t k0, uint32_t k1)
 {
     const uint64_t warp = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const uint32_t lane = threadIdx.x & 31u;
-    if (warp >= (uint64_t)NW32 * W) return;
-    const uint32_t w = (uint32_t)(warp % W), wq = (uint32_t)(warp / W);
+    if (warp >= (uint64_t)NW32 * W * clones) return;
+    const uint32_t w = (uint32_t)(warp % W), c = (uint32_t)((warp / W) % clones), wq = (uint32_t)(warp / ((uint64_t)W * clones));
     const uint64_t i = 32ull * wq + lane;
     uint64_t sigma = 0;
-    if (i < N) {
+    if (i < N && !aligned) {
         uint32_t x[4];
-        philox4x32_10((uint32_t)i, w, 0u, 1u << 24, k0, k1, x);
+        philox4x32_10((uint32_t)i, word0 + w + c * SK_CLONE_STRIDE, 0u, 1u << 24, k0, k1, x);
         sigma = (uint64_t)x[0] | ((uint64_t)x[1] << 32);
     }
     uint32_t mine0 = 0, mine1 = 0;
@@ -116,8 +119,9 @@ __global__ void __launch_bounds__(256) k_sk_init_spins(uint32_t *__restrict__ sb
         const uint32_t v1 = __ballot_sync(0xFFFFFFFFu, (sigma >> (b + 32)) & 1ull);
         if (lane == (uint32_t)b) { mine0 = v0; mine1 = v1; }
     }
-    sbits[(64ull * w + lane) * NW32 + wq] = mine0;
-    sbits[(64ull * w + 32 + lane) * NW32 + wq] = mine1;
+    const uint64_t l0 = 64ull * ((uint64_t)c * W + w) + lane;
+    sbits[l0 * NW32 + wq] = mine0;
+    sbits[(l0 + 32) * NW32 + wq] = mine1;
 }
 
 // ---------------------------------------------------------------------------------------- the sweep
@@ -126,7 +130,7 @@ __global__ void __launch_bounds__(256) k_sk_init_spins(uint32_t *__restrict__ sb
 __global__ void __launch_bounds__(SK_THREADS)
 k_sk_sweep(const uint32_t *__restrict__ rows, int16_t *__restrict__ Hg, uint32_t *__restrict__ sbits,
            const uint64_t *__restrict__ thr, uint32_t N, uint32_t NW32, uint32_t mz /* thr[m] = 0 for m >= mz */,
-           uint64_t sweep0, uint32_t nsweeps, uint32_t k0, uint32_t k1)
+           uint32_t lanes_w, uint32_t word0, uint64_t sweep0, uint32_t nsweeps, uint32_t k0, uint32_t k1)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const uint32_t nw32p = sk_nw32p(NW32);
@@ -136,9 +140,9 @@ k_sk_sweep(const uint32_t *__restrict__ rows, int16_t *__restrict__ Hg, uint32_t
     volatile uint32_t *ctl = sp + NW32;
 
     const uint32_t lane_g = blockIdx.x;
-    const uint32_t w = lane_g >> 6;
+    const uint32_t w = word0 + ((lane_g % lanes_w) >> 6) + (lane_g / lanes_w) * SK_CLONE_STRIDE;   // virtual word of the uniforms
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-    const uint32_t *myrows = rows + (uint64_t)lane_g * N * NW32;
+    const uint32_t *myrows = rows + (uint64_t)(lane_g % lanes_w) * N * NW32;
     int16_t *myH = Hg + (uint64_t)lane_g * 32u * NW32;
     uint32_t *mysp = sbits + (uint64_t)lane_g * NW32;
 
@@ -242,7 +246,7 @@ __global__ void __launch_bounds__(256) k_sk_energy(const int16_t *__restrict__ H
 
 // D_lane = popcount(sbits_now[lane] ^ sbits_slot[lane])
 __global__ void __launch_bounds__(256) k_sk_correlation(const uint32_t *__restrict__ a, const uint32_t *__restrict__ b,
-                                                        uint32_t NW32, unsigned long long *__restrict__ out)
+                                                        uint32_t NW32, unsigned long long *__restrict__ out, int accumulate)
 {
     __shared__ uint32_t part[8];
     const uint32_t lane_g = blockIdx.x;
@@ -255,7 +259,7 @@ __global__ void __launch_bounds__(256) k_sk_correlation(const uint32_t *__restri
     if (threadIdx.x == 0) {
         uint32_t tot = 0;
         for (uint32_t q = 0; q < blockDim.x / 32; ++q) tot += part[q];
-        out[lane_g] = tot;
+        out[lane_g] = accumulate ? out[lane_g] + tot : tot;
     }
 }
 
@@ -272,11 +276,11 @@ int sg_sk_create_impl(sg_sim *h)
     cudaStream_t st = sgx_stream();
     const uint64_t N = h->N;
     const uint32_t W = h->W, NW32 = sk_nw32(N);
-    const uint64_t lanes = 64ull * W;
+    const uint64_t lanes = h->lanes, lanes_w = 64ull * W;
     h->M = N * (N - 1) / 2;
     h->spin_words = lanes * NW32 / 2;   // u32 words, lanes even -> whole u64 count
     SKDevice &d = h->sk;
-    d.rows = dev_alloc<uint32_t>(h, lanes * N * NW32);
+    d.rows = dev_alloc<uint32_t>(h, lanes_w * N * NW32);
     d.H = dev_alloc<int16_t>(h, lanes * 32ull * NW32);
     d.spin = dev_alloc<uint64_t>(h, h->spin_words);
     d.thr = dev_alloc<uint64_t>(h, N);
@@ -289,21 +293,20 @@ int sg_sk_create_impl(sg_sim *h)
     if (!upload(d.thr, h->thr_host, st)) return SG_ECUDA;
     const size_t smem = sk_smem_bytes(NW32);
     if (smem > 227 * 1024) { sg_set_error("SK: N too large for the shared-memory field array"); return SG_EINVAL; }
-    if (!cuda_ok(cudaFuncSetAttribute(k_sk_sweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "SK smem attribute"))
-        return SG_ECUDA;
     {
         const uint64_t warps = N * NW32 * W;
-        k_sk_init_rows<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, st>>>(d.rows, N, NW32, W, h->key.k0, h->key.k1);
+        k_sk_init_rows<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, st>>>(d.rows, N, NW32, W, h->word0, h->key.k0, h->key.k1);
         SK_LAUNCH_CHECK();
     }
     {
-        const uint64_t warps = (uint64_t)NW32 * W;
-        k_sk_init_spins<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, st>>>((uint32_t *)d.spin, N, NW32, W, h->key.k0, h->key.k1);
+        const uint64_t warps = (uint64_t)NW32 * W * h->clones;
+        k_sk_init_spins<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, st>>>((uint32_t *)d.spin, N, NW32, W, h->clones, h->word0,
+                                                                              h->aligned ? 1 : 0, h->key.k0, h->key.k1);
         SK_LAUNCH_CHECK();
     }
     {
         dim3 grid((unsigned)((N + 255) / 256), (unsigned)lanes);
-        k_sk_init_fields<<<grid, 256, 0, st>>>(d.rows, (const uint32_t *)d.spin, d.H, N, NW32);
+        k_sk_init_fields<<<grid, 256, 0, st>>>(d.rows, (const uint32_t *)d.spin, d.H, N, NW32, (uint32_t)lanes_w);
         SK_LAUNCH_CHECK();
     }
     if (!cuda_ok(cudaStreamSynchronize(st), "sg_create (SK)")) return SG_ECUDA;
@@ -315,10 +318,13 @@ int sg_sk_sweep_impl(sg_sim *h, uint64_t n)
     cudaStream_t st = sgx_stream();
     const uint32_t NW32 = sk_nw32(h->N);
     const size_t smem = sk_smem_bytes(NW32);
+    // the limit is a property of the function, not of the handle: set it to this handle's need before every launch
+    // (another handle with a smaller N may have lowered it since)
+    if (!cuda_ok(cudaFuncSetAttribute(k_sk_sweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "SK smem attribute")) return SG_ECUDA;
     while (n) {
         const uint32_t chunk = (uint32_t)std::min<uint64_t>(n, 1u << 20);
-        k_sk_sweep<<<64u * h->W, SK_THREADS, smem, st>>>(h->sk.rows, h->sk.H, (uint32_t *)h->sk.spin, h->sk.thr, (uint32_t)h->N, NW32,
-                                                         h->sk.nthr_nz, h->sweep, chunk, h->key.k0, h->key.k1);
+        k_sk_sweep<<<(unsigned)h->lanes, SK_THREADS, smem, st>>>(h->sk.rows, h->sk.H, (uint32_t *)h->sk.spin, h->sk.thr, (uint32_t)h->N, NW32,
+                                                                 h->sk.nthr_nz, 64u * h->W, h->word0, h->sweep, chunk, h->key.k0, h->key.k1);
         SK_LAUNCH_CHECK();
         h->sweep += chunk;
         n -= chunk;
@@ -329,7 +335,7 @@ int sg_sk_sweep_impl(sg_sim *h, uint64_t n)
 int sg_sk_energy_impl(sg_sim *h, int64_t *out)
 {
     cudaStream_t st = sgx_stream();
-    const uint64_t lanes = 64ull * h->W;
+    const uint64_t lanes = h->lanes;
     k_sk_energy<<<(unsigned)lanes, 256, 0, st>>>(h->sk.H, (const uint32_t *)h->sk.spin, (uint32_t)h->N, sk_nw32(h->N),
                                                  (long long *)h->counts_dev);
     SK_LAUNCH_CHECK();
@@ -342,9 +348,9 @@ int sg_sk_energy_impl(sg_sim *h, int64_t *out)
 int sg_sk_correlation_impl(sg_sim *h, const uint64_t *slot_dev, uint64_t *out)
 {
     cudaStream_t st = sgx_stream();
-    const uint64_t lanes = 64ull * h->W;
+    const uint64_t lanes = h->lanes;
     k_sk_correlation<<<(unsigned)lanes, 256, 0, st>>>((const uint32_t *)h->sk.spin, (const uint32_t *)slot_dev, sk_nw32(h->N),
-                                                      (unsigned long long *)h->counts_dev);
+                                                      (unsigned long long *)h->counts_dev, 0);
     SK_LAUNCH_CHECK();
     if (!cuda_ok(cudaMemcpyAsync(out, h->counts_dev, lanes * 8, cudaMemcpyDeviceToHost, st), "sg_correlation") ||
         !cuda_ok(cudaStreamSynchronize(st), "sg_correlation"))
@@ -352,12 +358,22 @@ int sg_sk_correlation_impl(sg_sim *h, const uint64_t *slot_dev, uint64_t *out)
     return SG_OK;
 }
 
+// acc[lane] += D_lane(current, slot): the windowed protocol's accumulation, asynchronous
+int sg_sk_corr_accumulate_impl(sg_sim *h, const uint64_t *slot_dev, uint64_t *acc_dev)
+{
+    cudaStream_t st = sgx_stream();
+    k_sk_correlation<<<(unsigned)h->lanes, 256, 0, st>>>((const uint32_t *)h->sk.spin, (const uint32_t *)slot_dev, sk_nw32(h->N),
+                                                         (unsigned long long *)acc_dev, 1);
+    SK_LAUNCH_CHECK();
+    return SG_OK;
+}
+
 // lane-major bit arrays <-> site-major multispin words (host side; debug getters only)
 int sg_sk_get_spins_impl(sg_sim *h, const uint64_t *src_dev, uint64_t *out)
 {
     cudaStream_t st = sgx_stream();
-    const uint32_t NW32 = sk_nw32(h->N), W = h->W;
-    const uint64_t lanes = 64ull * W;
+    const uint32_t NW32 = sk_nw32(h->N), W = h->W * h->clones;      // lane groups per site, clone-major
+    const uint64_t lanes = h->lanes;
     std::vector<uint32_t> bits(lanes * NW32);
     if (!cuda_ok(cudaMemcpyAsync(bits.data(), src_dev, bits.size() * 4, cudaMemcpyDeviceToHost, st), "sg_get_spins") ||
         !cuda_ok(cudaStreamSynchronize(st), "sg_get_spins"))
@@ -372,15 +388,15 @@ int sg_sk_get_spins_impl(sg_sim *h, const uint64_t *src_dev, uint64_t *out)
 int sg_sk_set_spins_impl(sg_sim *h, const uint64_t *in)
 {
     cudaStream_t st = sgx_stream();
-    const uint32_t NW32 = sk_nw32(h->N), W = h->W;
-    const uint64_t lanes = 64ull * W;
+    const uint32_t NW32 = sk_nw32(h->N), W = h->W * h->clones;
+    const uint64_t lanes = h->lanes;
     std::vector<uint32_t> bits(lanes * NW32, 0u);
     for (uint64_t l = 0; l < lanes; ++l)
         for (uint64_t i = 0; i < h->N; ++i)
             if ((in[i * W + (l >> 6)] >> (l & 63)) & 1ull) bits[l * NW32 + (i >> 5)] |= 1u << (i & 31);
     if (!cuda_ok(cudaMemcpyAsync(h->sk.spin, bits.data(), bits.size() * 4, cudaMemcpyHostToDevice, st), "sg_set_spins")) return SG_ECUDA;
     dim3 grid((unsigned)((h->N + 255) / 256), (unsigned)lanes);
-    k_sk_init_fields<<<grid, 256, 0, st>>>(h->sk.rows, (const uint32_t *)h->sk.spin, h->sk.H, h->N, NW32);
+    k_sk_init_fields<<<grid, 256, 0, st>>>(h->sk.rows, (const uint32_t *)h->sk.spin, h->sk.H, h->N, NW32, 64u * h->W);
     SK_LAUNCH_CHECK();
     if (!cuda_ok(cudaStreamSynchronize(st), "sg_set_spins")) return SG_ECUDA;
     return SG_OK;

@@ -19,6 +19,7 @@
 // it misses L2, a whole line from HBM.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdlib>
 #include <string>
 
@@ -142,18 +143,13 @@ struct Streams {
             }
         }
     }
-    // a value that depends on every load above and can never equal PIN_IMPOSSIBLE
-    __device__ __forceinline__ uint32_t pin() const
+    // A value that can never equal PIN_IMPOSSIBLE and is known only when the last stream loads have returned: the
+    // last index and coupling loads of both runs (loads return in order per thread) and the two per-site loads.
+    __device__ __forceinline__ uint32_t pin(uint32_t site, uint32_t rp) const
     {
-        uint32_t a = 0xFFFFFFFFu;
-        uint64_t j = 0;
-#pragma unroll
-        for (int k = 0; k < IT; ++k) {
-            a &= nbT[k] & nbX[k];
-#pragma unroll
-            for (int g = 0; g < G; ++g) j |= jw[k].v[g];
-        }
-        return a & ((uint32_t)(j >> 32) | 0x7FFFFFFFu);
+        uint32_t a = nbT[IT - 1] & nbX[IT - 1] & nbT[0] & nbX[0];     // a position (< 2^31 - 2) or SG_NONE
+        a &= (uint32_t)(jw[IT - 1].v[G - 1] >> 32) | (uint32_t)(jw[0].v[0] >> 32) | site | rp | 0x7FFFFFFFu;
+        return a;
     }
     // the gather part: x_e = spin[neighbour] (^ coupling) into shared memory; all gathers in flight before the first store
     __device__ __forceinline__ void gather(const uint64_t *spin, uint32_t W, uint32_t w0, uint64_t *sT, uint64_t *sX) const
@@ -239,8 +235,9 @@ struct SweepArgs {
     const SGHdr *hdr;
     uint64_t thr[32];                 // thr[k], k = 0..31 (0 beyond dmax): read from the constant bank
     uint32_t slice0, nslices;         // of the colour class
-    uint32_t W, NG;                   // words per site, word groups (W / G)
-    uint32_t sweep_lo, sweep_hi, k0, k1;
+    uint32_t W, NG, word0;            // words per site, word groups (W / G), first word of the instance (multiple of 4)
+    uint32_t sweep_lo, sweep_hi;
+    uint32_t rk[20];                  // Philox round keys (k0 + r*0x9E3779B9, k1 + r*0xBB67AE85), r = 0..9
     uint32_t reverse;
 };
 
@@ -272,7 +269,7 @@ __global__ void __launch_bounds__(SG_BT, MINB) k_vb_sweep(const __grid_constant_
 
     // r = x_{w&3} of P(site, w>>2, sweep, tag 0): the ten Philox rounds run while the stream loads are in flight
     uint32_t x[4];
-    philox4x32_10(site, w0 >> 2, a.sweep_lo, a.sweep_hi, a.k0, a.k1, x);
+    philox4x32_10_keys(site, (a.word0 + w0) >> 2, a.sweep_lo, a.sweep_hi, a.rk, x);
     // thr[k] is non-increasing in k, so r < thr[kk] <=> kk <= kall := #{k >= 1 : r < thr[k]} (thr[k] = 0 beyond dmax)
     uint32_t kall[G];
 #pragma unroll
@@ -289,7 +286,7 @@ __global__ void __launch_bounds__(SG_BT, MINB) k_vb_sweep(const __grid_constant_
     // (ptxas hoists the wait above every global load that no thread exit separates from it; this exit is never
     // taken -- see PIN_IMPOSSIBLE -- and depends on every stream load, which pins them all in front of the wait;
     // tests/test_host_logic.py checks the order in the SASS)
-    if (st.pin() == PIN_IMPOSSIBLE) return;
+    if (st.pin(site, rp) == PIN_IMPOSSIBLE) return;
     griddep_wait();
     griddep_launch_dependents();
 
@@ -368,12 +365,12 @@ k_vb_unsat(const uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, co
 
 // ------------------------------------------------------------------------------------ couplings
 // O3 + gauge: the coupling entry x of the site at position p towards position nb, edge e = jeid[x], gets
-// J[x*W + w] = kappa_e[w] ^ eps[p*W + w] ^ eps[nb*W + w], kappa_e[w] = x0 | x1<<32 of P(e, w, 0, tag 2).
+// J[x*W + w] = kappa_e[w] ^ eps[p*W + w] ^ eps[nb*W + w], kappa_e[w] = x0 | x1<<32 of P(e, word0 + w, 0, tag 2).
 // One thread per site, every X entry and every word in turn (runs once per sg_create).
 __global__ void __launch_bounds__(SG_BT)
 k_init_vb_couplings(uint64_t *__restrict__ J, const uint64_t *__restrict__ eps, const uint32_t *__restrict__ col,
                     const uint32_t *__restrict__ jeid, const uint32_t *__restrict__ rp_s, const SGHdr *__restrict__ hdr,
-                    uint32_t nslices, uint32_t W, uint32_t k0, uint32_t k1)
+                    uint32_t nslices, uint32_t W, uint32_t word0, uint32_t k0, uint32_t k1)
 {
     const uint32_t slice = blockIdx.x * WARPS + (threadIdx.x >> 5), lane = threadIdx.x & 31u;
     if (slice >= nslices) return;
@@ -388,23 +385,24 @@ k_init_vb_couplings(uint64_t *__restrict__ J, const uint64_t *__restrict__ eps, 
         const uint32_t e = jeid[xi];
         for (uint32_t w = 0; w < W; ++w) {
             uint32_t x[4];
-            philox4x32_10(e, w, 0u, 2u << 24, k0, k1, x);
+            philox4x32_10(e, word0 + w, 0u, 2u << 24, k0, k1, x);
             J[xi * W + w] = ((uint64_t)x[0] | ((uint64_t)x[1] << 32)) ^ eps[p * W + w] ^ eps[nb * W + w];
         }
     }
 }
 
 template <int G, bool WIDE, bool W1, int MINB>
-int launch(const VBDevice &d, const VBClass &c, uint32_t W, uint64_t sweep, SGSeed key, bool reverse, cudaStream_t st)
+int launch(const VBDevice &d, const VBClass &c, uint32_t W, uint32_t word0, uint64_t sweep, SGSeed key, bool reverse, cudaStream_t st)
 {
     if (d.cap > (uint32_t)Cap<G>::value) { sg_set_error("k_vb_sweep: the slice budget of the instance exceeds the kernel's"); return SG_EINVAL; }
     SweepArgs a;
     a.spin = d.spin; a.J = d.J; a.col = d.col; a.orig_s = d.orig_s; a.rp_s = d.rp_s; a.hdr = d.hdr;
     for (int k = 0; k < 32; ++k) a.thr[k] = d.thr_host[k];
     a.slice0 = (uint32_t)c.slice0; a.nslices = (uint32_t)c.nslices;
-    a.W = W; a.NG = W / G;
+    a.W = W; a.NG = W / G; a.word0 = word0;
     a.sweep_lo = (uint32_t)sweep; a.sweep_hi = (uint32_t)(sweep >> 32) /* tag 0 */;
-    a.k0 = key.k0; a.k1 = key.k1; a.reverse = reverse ? 1u : 0u;
+    for (uint32_t r = 0; r < 10; ++r) { a.rk[2 * r] = key.k0 + r * 0x9E3779B9u; a.rk[2 * r + 1] = key.k1 + r * 0xBB67AE85u; }
+    a.reverse = reverse ? 1u : 0u;
     const uint64_t jobs = c.nslices * a.NG;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)((jobs + WARPS - 1) / WARPS));
@@ -432,7 +430,7 @@ bool force_wide() { return std::getenv("SG_FORCE_WIDE") != nullptr; }
 
 }  // namespace
 
-int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint64_t N, uint64_t nJ, uint32_t W, uint64_t sweep, SGSeed key,
+int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint64_t N, uint64_t nJ, uint32_t W, uint32_t word0, uint64_t sweep, SGSeed key,
                        bool reverse, cudaStream_t st)
 {
     if (c.n == 0) return SG_OK;
@@ -441,16 +439,16 @@ int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint64_t N, uint64_t
     if (c.nslices * (uint64_t)(W / G) >= (1ull << 31)) { sg_set_error("sgk_vb_sweep_class: class too large"); return SG_EINVAL; }
     if (!wide) {
         switch (G) {
-        case 1: return W == 1 ? launch<1, false, true, SG_MINB1>(d, c, W, sweep, key, reverse, st)
-                              : launch<1, false, false, SG_MINB1>(d, c, W, sweep, key, reverse, st);
-        case 2: return launch<2, false, false, 6>(d, c, W, sweep, key, reverse, st);
-        default: return launch<4, false, false, 4>(d, c, W, sweep, key, reverse, st);
+        case 1: return W == 1 ? launch<1, false, true, SG_MINB1>(d, c, W, word0, sweep, key, reverse, st)
+                              : launch<1, false, false, SG_MINB1>(d, c, W, word0, sweep, key, reverse, st);
+        case 2: return launch<2, false, false, 6>(d, c, W, word0, sweep, key, reverse, st);
+        default: return launch<4, false, false, 4>(d, c, W, word0, sweep, key, reverse, st);
         }
     }
     switch (G) {
-    case 1: return launch<1, true, false, SG_MINB1>(d, c, W, sweep, key, reverse, st);
-    case 2: return launch<2, true, false, 6>(d, c, W, sweep, key, reverse, st);
-    default: return launch<4, true, false, 4>(d, c, W, sweep, key, reverse, st);
+    case 1: return launch<1, true, false, SG_MINB1>(d, c, W, word0, sweep, key, reverse, st);
+    case 2: return launch<2, true, false, 6>(d, c, W, word0, sweep, key, reverse, st);
+    default: return launch<4, true, false, 4>(d, c, W, word0, sweep, key, reverse, st);
     }
 }
 
@@ -472,12 +470,12 @@ int sgk_vb_unsat(const VBDevice &d, uint64_t N, uint64_t nJ, uint32_t W, uint64_
     return SG_OK;
 }
 
-int sgk_init_vb_couplings(const VBDevice &d, const uint32_t *jeid, uint32_t W, SGSeed key, cudaStream_t st)
+int sgk_init_vb_couplings(const VBDevice &d, const uint32_t *jeid, uint32_t W, uint32_t word0, SGSeed key, cudaStream_t st)
 {
     const uint64_t nslices = d.nslices;
     if (nslices == 0) return SG_OK;
     k_init_vb_couplings<<<(unsigned)((nslices + WARPS - 1) / WARPS), SG_BT, 0, st>>>(d.J, d.eps, d.col, jeid, d.rp_s, d.hdr, (uint32_t)nslices, W,
-                                                                                     key.k0, key.k1);
+                                                                                     word0, key.k0, key.k1);
     sgk_count_launch();
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { sg_set_error(std::string("k_init_vb_couplings launch failed: ") + cudaGetErrorString(e)); return SG_ECUDA; }

@@ -108,7 +108,43 @@ def window_index(time: int) -> int:
     return m - 1 if t4 == 1 << m else m      # time^4 in (2^m, 2^(m+1)]  <=>  time in (t_m, t_{m+1}]
 
 
-def run_windowed(sim, total_sweeps: int, tws=(4, 16, 64, 256, 1024, 4096)):
+def tritone_index(time: int) -> int:
+    """Index of the tritone lump of the total time tw + t (data with the same value of
+    floor(ln((t + tw)/4) / (0.5 ln 2)) are lumped together, e.g. tw + t = {4, 5}).  Integer-exact:
+    floor(2 log2(time/4)) = floor(log2(time^2)) - 4."""
+    if time < 1:
+        raise ValueError("time must be >= 1")
+    return (time * time).bit_length() - 1 - 4
+
+
+def run_windowed_device(sim, total_sweeps: int, tws=(4, 16, 64, 256, 1024, 4096), binning=window_index):
+    """The windowed protocol with the bookkeeping on the device (sg_corr_configure / _accumulate / _fetch): after every
+    sweep ONE asynchronous call adds D against every stored tw to that tw's current bin; the host fetches once at the
+    end.  Same result as run_windowed (the reference harness, which works on any object with sweep/snapshot/correlation):
+    {(tw, m): (sum of D per lane, number of times)}."""
+    tws = [tw for tw in tws if tw <= total_sweeps]
+    slot_of = {tw: k for k, tw in enumerate(tws)}
+    m0 = binning(1)
+    nb = binning(total_sweeps) - m0 + 1                     # bins per tw
+    sim.corr_configure(max(1, nb * len(tws)))
+    for time in range(1, total_sweeps + 1):
+        sim.sweep(1)
+        active = [tw for tw in tws if time > tw]
+        if active:
+            sim.corr_accumulate([slot_of[tw] for tw in active], [slot_of[tw] * nb + binning(time) - m0 for tw in active])
+        if time in slot_of:
+            sim.snapshot(slot_of[time])
+    acc, hits = sim.corr_fetch(0, max(1, nb * len(tws)))
+    out = {}
+    for tw in tws:
+        for b in range(nb):
+            q = slot_of[tw] * nb + b
+            if hits[q]:
+                out[(tw, b + m0)] = (acc[q].copy(), int(hits[q]))
+    return out
+
+
+def run_windowed(sim, total_sweeps: int, tws=(4, 16, 64, 256, 1024, 4096), binning=window_index):
     """The paper's measurement protocol on any object with sweep/snapshot/correlation (the binding's Sim or the oracle's
     handle): snapshot at every waiting time tw (tw = 2^2, 2^4, ..., 2^12), then after EVERY sweep count D
     against every stored tw and add it to the bin of the total time tw + t (window_index).  Returns
@@ -123,7 +159,7 @@ def run_windowed(sim, total_sweeps: int, tws=(4, 16, 64, 256, 1024, 4096)):
         sim.sweep(1)
         for tw in tws:
             if time > tw:
-                key = (tw, window_index(time))
+                key = (tw, binning(time))
                 d = np.asarray(sim.correlation(slot_of[tw]), dtype=np.uint64)
                 if key in out:
                     out[key] = (out[key][0] + d, out[key][1] + 1)

@@ -111,3 +111,103 @@ def test_sk_long_run_energy_consistency(sg):
     pr = np.array([[i, j] for i in range(N) for j in range(i + 1, N)])
     E = -(K * S[pr[:, 0]] * S[pr[:, 1]]).sum(axis=0)
     assert np.array_equal(g.energy(), E)
+
+
+@pytest.mark.parametrize("N,T,seed,W,aligned", [(256, 0.4, 21, 1, True), (100, 0.5, 22, 2, True), (512, 0.6, 23, 1, False)])
+def test_sk_protocol_of_the_si(sg, oracle_mod, N, T, seed, W, aligned):
+    """PAPER.md:231-233, :244: two clones per coupling set, all-aligned start, T in {0.4, 0.5, 0.6}, waiting time tw = 3;
+    every sweep compared with the oracle, energies and the counts against the tw = 3 snapshot as well."""
+    g = sg.Sim(sg.SG_MODEL_SK, N, 0.0, T, seed, W, n_clones=2, aligned_start=aligned)
+    o = oracle_mod.Oracle(oracle_mod.SK, N, 0.0, T, seed, W, n_clones=2, aligned_start=aligned)
+    assert g.lanes == o.lanes == 128 * W
+    _same(g, o)
+    if aligned:
+        assert np.all(g.spins() == 0)
+    assert np.array_equal(g.couplings(), o.couplings())
+    assert np.array_equal(g.energy(), o.energy())
+    g.sweep(3); o.sweep(3)
+    g.snapshot(0); o.snapshot(0)
+    for _ in range(5):
+        g.sweep(1); o.sweep(1)
+        _same(g, o)
+        assert np.array_equal(g.energy(), o.energy())
+        assert np.array_equal(g.correlation(0), o.correlation(0))
+    # clone 0 is the plain run of the same instance
+    p = sg.Sim(sg.SG_MODEL_SK, N, 0.0, T, seed, W, aligned_start=aligned)
+    p.sweep(8)
+    assert np.array_equal(p.spins(), g.spins()[:, :W])
+
+
+def test_sk_word_offset(sg, oracle_mod):
+    """sg_options.word0: words 4..7 of an 8-word instance from their own handle."""
+    N, T = 160, 0.6
+    full = sg.Sim(sg.SG_MODEL_SK, N, 0.0, T, 31, 8)
+    part = sg.Sim(sg.SG_MODEL_SK, N, 0.0, T, 31, 4, word0=4)
+    o = oracle_mod.Oracle(oracle_mod.SK, N, 0.0, T, 31, 4, word0=4)
+    full.sweep(4); part.sweep(4); o.sweep(4)
+    assert np.array_equal(part.spins(), full.spins()[:, 4:])
+    assert np.array_equal(part.spins(), o.spins())
+    assert np.array_equal(part.energy(), full.energy()[256:])
+
+
+def test_two_sk_handles_of_different_size(sg, oracle_mod):
+    """The dynamic shared-memory limit of the sweep kernel belongs to the function, not to a handle: creating and
+    sweeping a small instance must not break a larger one that needs more than 48 KiB."""
+    big = sg.Sim(sg.SG_MODEL_SK, 12000, 0.0, 0.6, 41, 1)
+    small = sg.Sim(sg.SG_MODEL_SK, 64, 0.0, 0.6, 42, 1)
+    small.sweep(2)
+    big.sweep(1)
+    small.sweep(1)
+    big.sweep(1)
+    E = big.energy()
+    assert E.shape == (64,) and np.all(E < 0)
+    o = oracle_mod.Oracle(oracle_mod.SK, 64, 0.0, 0.6, 42, 1)
+    o.sweep(3)
+    assert np.array_equal(small.spins(), o.spins())
+
+
+def test_sk_largest_size(sg, oracle_mod):
+    """N = 2^15, the largest size of the paper's SK runs and the limit of int16 local fields (Q22).  The
+    GPU runs two sweeps from the aligned start; the oracle (from-scratch fields) replays three windows of the second
+    sweep -- its first, a middle and its last 512 site updates -- from the mixed state in which the sites below the
+    window carry the GPU's new values and the others its old ones.  Plus: the incremental int16 fields after the sweeps
+    equal fields recomputed from scratch (energy before and after re-importing the configuration)."""
+    N, T, K = 1 << 15, 0.4, 512
+    from concurrent.futures import ThreadPoolExecutor
+
+    with ThreadPoolExecutor(max_workers=2) as ex:
+        fo = ex.submit(lambda: oracle_mod.Oracle(oracle_mod.SK, N, 0.0, T, 51, 1, aligned_start=True))
+        fg = ex.submit(lambda: sg.Sim(sg.SG_MODEL_SK, N, 0.0, T, 51, 1, aligned_start=True))
+        o, g = fo.result(), fg.result()
+    g.sweep(1)
+    old = g.spins()
+    g.sweep(1)
+    new = g.spins()
+    assert 0 < int((old != new).sum()) < N
+    o.set_sweep_count(1)
+    for i0 in (0, N // 2 - 100, N - K):
+        mixed = old.copy()
+        mixed[:i0] = new[:i0]
+        o.set_spins(mixed)
+        o.sk_update_range(i0, i0 + K)
+        assert np.array_equal(o.spins()[i0:i0 + K], new[i0:i0 + K]), i0
+    E = g.energy()
+    g.set_spins(new)                       # recomputes every local field from scratch
+    assert np.array_equal(g.energy(), E)
+    g.sweep(1)                             # and the dynamics goes on from there
+    assert g.sweep_count == 3
+
+
+def test_sk_windowed_tritone_protocol(sg, oracle_mod):
+    """SK as the SI measures it: two clones, aligned start, tw = 3, every sweep counted against the tw = 3 snapshot and
+    lumped in tritone intervals of tw + t, accumulated on the device."""
+    from paper_1906_11195_b200 import workloads as wl
+
+    N, S = 128, 60
+    g = sg.Sim(sg.SG_MODEL_SK, N, 0.0, 0.5, 61, 1, n_clones=2, aligned_start=True)
+    o = oracle_mod.Oracle(oracle_mod.SK, N, 0.0, 0.5, 61, 1, n_clones=2, aligned_start=True)
+    rd = wl.run_windowed_device(g, S, tws=(3,), binning=wl.tritone_index)
+    ro = wl.run_windowed(o, S, tws=(3,), binning=wl.tritone_index)
+    assert rd.keys() == ro.keys() and len(rd) >= 6
+    for k in rd:
+        assert rd[k][1] == ro[k][1] and np.array_equal(rd[k][0], ro[k][0]), k

@@ -350,18 +350,29 @@ def test_rrbg_full_size_late_sweep(sg, oracle_mod):
     _late_sweep_check(g, o, 30)
 
 
-def test_windowed_protocol_matches_oracle(sg, oracle_mod):
+@pytest.mark.parametrize("model,N,W,binning", [(2, 4096, 2, "minor_third"), (0, 3000, 3, "minor_third"), (0, 2000, 1, "tritone")])
+def test_windowed_protocol_matches_oracle(sg, oracle_mod, model, N, W, binning):
     """The paper's measurement protocol (snapshots at tw = 4, 16, 64; D against every tw after every sweep, binned in
-    minor-third intervals of tw + t) gives the same exact sums on the GPU path and on the oracle."""
-    from paper_1906_11195_b200.workloads import run_windowed
+    minor-third intervals of tw + t, or in the SK section's tritone lumps, :233): the device-side
+    accumulation (sg_corr_*: one asynchronous multi-slot pass per sweep, one fetch at the end) gives the same exact
+    sums as the reference harness on the oracle, and as the reference harness on the GPU (one count per tw and sweep)."""
+    from paper_1906_11195_b200 import workloads as wl
 
-    N, S = 4096, 100
-    g = sg.Sim(sg.SG_MODEL_RRBG, N, 0.0, 1.2149, 5, 2)
-    o = oracle_mod.Oracle(oracle_mod.RRBG, N, 0.0, 1.2149, 5, 2)
-    rg, ro = run_windowed(g, S), run_windowed(o, S)
-    assert rg.keys() == ro.keys() and len(rg) > 20
-    for k in rg:
-        assert rg[k][1] == ro[k][1] and np.array_equal(rg[k][0], ro[k][0]), k
+    S = 100
+    rule = wl.window_index if binning == "minor_third" else wl.tritone_index
+    c, T = (0.0, 1.2149) if model == 2 else (4.0, 1.0)
+    g = sg.Sim(model, N, c, T, 5, W)
+    g2 = sg.Sim(model, N, c, T, 5, W)
+    o = oracle_mod.Oracle(model, N, c, T, 5, W)
+    rd, rg, ro = wl.run_windowed_device(g, S, binning=rule), wl.run_windowed(g2, S, binning=rule), wl.run_windowed(o, S, binning=rule)
+    assert rd.keys() == ro.keys() == rg.keys() and len(rd) > 15
+    for k in rd:
+        assert rd[k][1] == ro[k][1] == rg[k][1], k
+        assert np.array_equal(rd[k][0], ro[k][0]) and np.array_equal(rg[k][0], ro[k][0]), k
+    with pytest.raises(sg.SGError):
+        g.corr_accumulate([0, 1], [3, 3])                      # bins of one call must be distinct
+    with pytest.raises(sg.SGError):
+        g.corr_accumulate([9], [0])                            # slot never written
 
 
 @pytest.mark.parametrize("log2n,W,T,sweeps", [(12, 16, 0.6, 256), (12, 16, 1.0, 256), (12, 16, 1.4, 256), (16, 16, 0.6, 8), (16, 16, 1.4, 8),
@@ -381,3 +392,37 @@ def test_config5_sizes_and_temperatures(sg, oracle_mod, log2n, W, T, sweeps):
         assert np.array_equal(cg[k], co[k]), k
     _assert_same_state(g, o)
     assert np.array_equal(g.energy(), o.energy())
+
+
+@pytest.mark.parametrize("model,N,c,T", [(0, 6000, 4.0, 1.0), (2, 4096, 0.0, 1.2149)])
+def test_word_offset_shards_reproduce_the_whole_run(sg, oracle_mod, model, N, c, T):
+    """sg_options.word0 (Q24): the words of one instance split over several handles -- as over
+    several GPUs -- give exactly the columns of the single-handle run, and equal the oracle run with the same offset."""
+    full = sg.Sim(model, N, c, T, 17, 12)
+    parts = [sg.Sim(model, N, c, T, 17, 4, word0=4 * k) for k in range(3)]
+    o = oracle_mod.Oracle(model, N, c, T, 17, 4, word0=8)
+    full.snapshot(0); o.snapshot(0)
+    for p in parts:
+        p.snapshot(0)
+    full.sweep(5); o.sweep(5)
+    S, E, D = full.spins(), full.energy(), full.correlation(0)
+    for k, p in enumerate(parts):
+        p.sweep(5)
+        assert np.array_equal(p.spins(), S[:, 4 * k:4 * k + 4])
+        assert np.array_equal(p.energy(), E[256 * k:256 * k + 256])
+        assert np.array_equal(p.correlation(0), D[256 * k:256 * k + 256])
+        assert np.array_equal(p.couplings(), full.couplings()[:, 4 * k:4 * k + 4])
+    assert np.array_equal(parts[2].spins(), o.spins())
+    with pytest.raises(sg.SGError):
+        sg.Sim(model, N, c, T, 17, 4, word0=2)                     # not a multiple of 4
+    with pytest.raises(sg.SGError):
+        sg.Sim(model, N, c, T, 17, 1, n_clones=2)                  # clones are an SK option
+
+
+def test_aligned_start_vb(sg, oracle_mod):
+    g = sg.Sim(sg.SG_MODEL_VB, 5000, 4.0, 1.0, 19, 2, aligned_start=True)
+    o = oracle_mod.Oracle(oracle_mod.VB, 5000, 4.0, 1.0, 19, 2, aligned_start=True)
+    assert np.all(g.spins() == 0)
+    assert np.array_equal(g.energy(), o.energy())
+    g.sweep(4); o.sweep(4)
+    _assert_same_state(g, o)

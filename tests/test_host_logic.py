@@ -293,6 +293,27 @@ def test_window_index_is_the_minor_third_bin():
         assert abs(len(seen[m + 1]) / len(seen[m]) - 2 ** 0.25) < 0.15
 
 
+def test_tritone_index_is_the_papers_lump():
+    """"we lump together the data for the same value of floor(ln((t+tw)/4)/(0.5 ln 2)) ... e.g. we lump
+    together the t + tw = {4, 5} data"."""
+    import math
+
+    from paper_1906_11195_b200.workloads import tritone_index
+
+    assert tritone_index(4) == tritone_index(5) == 0 and tritone_index(6) == 1
+    for x in range(4, 20000):
+        v = math.log(x / 4) / (0.5 * math.log(2))
+        if abs(v - round(v)) > 1e-9:                      # away from the lump edges floating point is safe
+            assert tritone_index(x) == math.floor(v), x
+    for k in range(2, 40):                                # the edges that are integers: x = 2^k -> index 2k - 4
+        assert tritone_index(1 << k) == 2 * k - 4 and tritone_index((1 << k) - 1) == 2 * k - 5
+    sizes = {}
+    for x in range(4, 1 << 16):
+        sizes[tritone_index(x)] = sizes.get(tritone_index(x), 0) + 1
+    for m in range(14, 24):                               # lump widths grow by sqrt(2): "tritone" intervals
+        assert abs(sizes[m + 1] / sizes[m] - 2 ** 0.5) < 0.02
+
+
 def test_windowed_protocol_on_the_oracle(oracle_mod):
     """run_windowed against a direct recomputation from stored configurations (small N, the oracle as the simulator)."""
     from paper_1906_11195_b200.workloads import run_windowed, window_index
@@ -315,3 +336,35 @@ def test_windowed_protocol_on_the_oracle(oracle_mod):
     assert res.keys() == expect.keys()
     for k in res:
         assert res[k][1] == expect[k][1] and np.array_equal(res[k][0], expect[k][0]), k
+
+
+def test_sweep_kernels_read_no_spin_before_the_dependent_launch_wait(sg):
+    """The sweep launches are programmatic dependent launches: a CTA may start while the previous colour class is still
+    running, reads its read-only streams, and must not touch a spin word before `griddepcontrol.wait` (SASS: ACQBULK).
+    ptxas is kept from hoisting the wait above the stream loads by a never-taken exit (csrc/sg_vb_sweep.cu); this
+    test pins the resulting order in the shipped binary: in every k_vb_sweep instantiation, every global load in
+    front of ACQBULK is a read-only (.CONSTANT) load, there are at least four of them, the first plain load (a spin
+    word) and the only store come after it."""
+    import shutil
+    import subprocess
+
+    from paper_1906_11195_b200 import binding
+
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    sass = subprocess.run([cuobjdump, "-sass", binding.LIB_PATH], capture_output=True, text=True, check=True).stdout
+    funcs = re.split(r"\n\s*Function : ", sass)[1:]
+    sweeps = [f for f in funcs if "k_vb_sweep" in f.split("\n", 1)[0]]
+    assert len(sweeps) >= 6                                    # G = 1 (W = 1 and general), 2, 4, each narrow and wide
+    for f in sweeps:
+        name = f.split("\n", 1)[0]
+        ops = re.findall(r"/\*[0-9a-f]{4}\*/\s+(?:@!?U?P\d\s+)?([A-Z0-9_.]+)", f)
+        assert ops.count("ACQBULK") == 1, name
+        k = ops.index("ACQBULK")
+        before, after = ops[:k], ops[k + 1:]
+        loads_before = [o for o in before if o.startswith("LDG")]
+        assert len(loads_before) >= 4 and all(".CONSTANT" in o for o in loads_before), (name, loads_before)
+        assert not any(o.startswith(("STG", "ATOM", "RED")) for o in before), name
+        assert any(o.startswith("LDG") and ".CONSTANT" not in o for o in after), name      # the spin reads
+        assert sum(1 for o in after if o.startswith("STG")) >= 1, name

@@ -98,3 +98,21 @@ def test_sk_energy_bookkeeping(oracle_mod, T):
         if math.isinf(T):
             assert np.all(o.correlation(0) == (N if t % 2 else 0))
         Eprev = E
+
+
+def test_sk_sweep_is_the_ordered_composition_of_site_updates(oracle_mod):
+    """PAPER.md:233 "N single spin updates, performed in a fixed order": or_sk_update_range (used by the GPU tests to
+    check windows of the N = 2^15 sweep) composes to or_sweep."""
+    a = oracle_mod.Oracle(oracle_mod.SK, 64, 0.0, 0.6, 3, 2)
+    b = oracle_mod.Oracle(oracle_mod.SK, 64, 0.0, 0.6, 3, 2)
+    for t in range(3):
+        a.sweep(1)
+        b.sk_update_range(0, 20); b.sk_update_range(20, 21); b.sk_update_range(21, 64)
+        b.set_sweep_count(t + 1)
+        assert np.array_equal(a.spins(), b.spins())
+    c = oracle_mod.Oracle(oracle_mod.SK, 64, 0.0, 0.6, 3, 2)
+    c.sk_update_range(10, 30)                       # a different order is a different map
+    c.sk_update_range(0, 10); c.sk_update_range(30, 64)
+    a2 = oracle_mod.Oracle(oracle_mod.SK, 64, 0.0, 0.6, 3, 2)
+    a2.sweep(1)
+    assert not np.array_equal(a2.spins(), c.spins())
