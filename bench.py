@@ -38,8 +38,12 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--T", type=float, default=1.0)
-    ap.add_argument("--model", default="vb", choices=["vb", "sk", "rrbg"],
-                    help="sk: BASELINE.json configs[3] with --log2n 12 (absolute rate only); rrbg: the paper's own ensemble (SURVEY.md 8(f) rank 1), use --T 1.2149")
+    ap.add_argument("--model", default="vb", choices=["vb", "sk", "rrbg", "rrg"],
+                    help="sk: BASELINE.json configs[3] with --log2n 12 (absolute rate only); rrbg / rrg: the paper's own ensembles "
+                         "(SURVEY.md 8(f) rank 1), use --T 1.2149")
+    ap.add_argument("--windowed", type=int, default=0, metavar="S",
+                    help="also time the windowed protocol: sg_sweep(1) + one sg_corr_accumulate against S stored configurations per sweep")
+    ap.add_argument("--clones", type=int, default=1, help="SK: replicas that share the couplings (PAPER.md:233)")
     ap.add_argument("--log2n", type=int, default=24)
     ap.add_argument("--n-words", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -161,12 +165,12 @@ def run_ours(args):
     t0 = time.perf_counter()
     from paper_1906_11195_b200.workloads import Workload, shard
 
-    model = {"vb": sg.SG_MODEL_VB, "sk": sg.SG_MODEL_SK, "rrbg": sg.SG_MODEL_RRBG}[args.model]
+    model = {"vb": sg.SG_MODEL_VB, "sk": sg.SG_MODEL_SK, "rrbg": sg.SG_MODEL_RRBG, "rrg": sg.SG_MODEL_RRG}[args.model]
     wl = shard(Workload("bench", model, N, 4.0, args.T, 1, W, 0), rank, world)
-    sim = sg.Sim(wl.model, wl.N, wl.c, wl.T, wl.seed, wl.n_words)
+    sim = sg.Sim(wl.model, wl.N, wl.c, wl.T, wl.seed, wl.n_words, n_clones=args.clones)
     create_s = time.perf_counter() - t0
-    counts = np.zeros(64 * W, dtype=np.uint64)
-    energy = np.zeros(64 * W, dtype=np.int64)
+    counts = np.zeros(sim.lanes, dtype=np.uint64)
+    energy = np.zeros(sim.lanes, dtype=np.int64)
     sweep_ev = []
 
     def step(timed):
@@ -207,14 +211,14 @@ def run_ours(args):
         t = torch.tensor([ms, sweep_ms], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms, sweep_ms = float(t[0]), float(t[1])
-    updates_per_rank = N * 64 * W * SWEEPS_PER_STEP * args.steps
+    updates_per_rank = N * sim.lanes * SWEEPS_PER_STEP * args.steps
     value = updates_per_rank * world / (ms * 1e-3)
 
     # ---- e2e: the same step through the C-ABI with HOST buffers: the configuration goes in from pinned host
     # memory (sg_set_spins) and comes back (sg_get_spins) every step, as in the paper's flow
     e2e = None
     if not args.no_e2e:
-        host = torch.empty((N, W), dtype=torch.int64, pin_memory=True).numpy().view(np.uint64)
+        host = torch.empty((N, sim.groups), dtype=torch.int64, pin_memory=True).numpy().view(np.uint64)
         sim.spins(out=host)
         for _ in range(2):
             sim.set_spins(host); step(False); sim.spins(out=host)
@@ -231,8 +235,41 @@ def run_ours(args):
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             dt = float(t[0])
         e2e = {"value": updates_per_rank * world / dt, "unit": "spin updates/s",
-               "h2d_bytes_per_step": N * W * 8, "d2h_bytes_per_step": N * W * 8 + 2 * 64 * W * 8,
+               "h2d_bytes_per_step": N * sim.groups * 8, "d2h_bytes_per_step": N * sim.groups * 8 + 2 * sim.lanes * 8,
                "note": "sg_set_spins(pinned host) + step + sg_get_spins(pinned host) per step, wall clock"}
+    windowed = None
+    if args.windowed > 0:
+        # the paper's measurement protocol: after EVERY sweep count against every stored tw;
+        # here S stored configurations, the sums kept on the device (sg_corr_accumulate), fetched once at the end
+        S = args.windowed
+        for k in range(S):
+            sim.snapshot(k)
+            sim.sweep(1)
+        sim.corr_configure(S)
+        slots, bins = list(range(S)), list(range(S))
+        nsw = 64
+
+        def timed(with_acc):
+            sync_all()
+            a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(nsw):
+                sim.sweep(1)
+                if with_acc:
+                    sim.corr_accumulate(slots, bins)
+            b_.record()
+            sync_all()
+            return a.elapsed_time(b_) / nsw
+
+        timed(True)
+        t_with, t_without = timed(True), timed(False)
+        acc, hits = sim.corr_fetch(0, S)
+        assert int(hits[0]) == 3 * nsw - nsw and np.all(acc[0] > 0)
+        bytes_per_sweep = (8 + 8 * S) * N * W
+        windowed = {"slots": S, "ms_per_sweep_with_accumulate": t_with, "ms_per_sweep_without": t_without,
+                    "accumulate_ms_per_sweep": t_with - t_without, "algorithmic_bytes_per_sweep": bytes_per_sweep,
+                    "accumulate_gb_per_s": bytes_per_sweep / ((t_with - t_without) * 1e-3) / 1e9,
+                    "note": "one asynchronous sg_corr_accumulate per sweep: (8 + 8 S) bytes per site-word in passes of up to 3 slots"}
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -245,7 +282,7 @@ def run_ours(args):
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "u64", "data": "synthetic",
         "config": {"workload": (f"VB N=2^{args.log2n} c=4 W={W} T={args.T} seed=1+rank (BASELINE.json configs[2])" if args.model == "vb"
-                                else f"RRBG degree 4 N=2^{args.log2n} W={W} T={args.T} seed=1+rank (the paper's ensemble, PAPER.md:260; not the headline workload)" if args.model == "rrbg"
+                                else f"{args.model.upper()} degree 4 N=2^{args.log2n} W={W} T={args.T} seed=1+rank (the paper's ensemble, PAPER.md:75, :260; not the headline workload)" if args.model in ("rrbg", "rrg")
                                 else f"SK N=2^{args.log2n} W={W} T={args.T} seed=1+rank (BASELINE.json configs[3]; dependency-latency bound, roofline fields not meaningful)"),
                    "step": f"sg_sweep({SWEEPS_PER_STEP}) + sg_snapshot + sg_correlation + sg_energy",
                    "l2": "inputs larger than L2: every sweep streams 777 MiB of couplings+indices+labels and reads/writes the 128 MiB spin array (L2 126 MiB); no flush needed",
@@ -257,6 +294,8 @@ def run_ours(args):
                      "sweep_share_of_step": sweep_ms / ms},
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
     }
+    if windowed:
+        out["windowed"] = windowed
     tr = os.path.join(ROOT, "profiles", "traffic.json")
     headline = args.model == "vb" and args.log2n == 24 and W == 1
     if os.path.exists(tr) and headline:      # ncu dram bytes of one sweep of exactly this workload (profiles/r01_sweep.md)

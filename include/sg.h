@@ -29,7 +29,7 @@ extern "C" {
 
 typedef struct sg_sim sg_sim; /* opaque; owns every device and host buffer of one simulation */
 
-enum { SG_MODEL_VB = 0, SG_MODEL_SK = 1, SG_MODEL_RRBG = 2 };
+enum { SG_MODEL_VB = 0, SG_MODEL_SK = 1, SG_MODEL_RRBG = 2, SG_MODEL_RRG = 3 };
 enum { SG_OK = 0, SG_EINVAL = -1, SG_ENOMEM = -2, SG_ECUDA = -3, SG_ESLOT = -4 };
 #define SG_MAX_SLOTS 64
 
@@ -44,6 +44,9 @@ enum { SG_OK = 0, SG_EINVAL = -1, SG_ENOMEM = -2, SG_ECUDA = -3, SG_ESLOT = -4 }
  *                        bipartite graph of degree 4: halves {0..N/2-1} and {N/2..N-1},
  *                        four clash-free random permutations of one half onto the other (O2b), hence
  *                        exactly two colour classes; N even and >= 8; c is ignored.
+ *           SG_MODEL_RRG: the same Hamiltonian on a random regular graph of degree 4 that is not bipartite (the ensemble of the
+ *                        main text; Fig. S3, shows that bipartition is irrelevant): the first
+ *                        simple graph of the pairing model (O2c); first-fit colour classes; 8 <= N < 2^30; c ignored.
  *   N       number of sites, 2 <= N < 2^31 - 2 (SK: N <= 32768 so that int16 local fields are exact).
  *   c       mean degree (VB), c >= 0 and M <= N(N-1)/2.
  *   T       temperature, 0 <= T <= +inf (T = 0 and T = inf are legal).
@@ -196,7 +199,7 @@ void sg_host_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t
  * uses the original label (Q15).
  */
 typedef struct sg_host_graph sg_host_graph;
-/* model: SG_MODEL_VB or SG_MODEL_RRBG; NULL on bad arguments */
+/* model: SG_MODEL_VB, SG_MODEL_RRBG or SG_MODEL_RRG; NULL on bad arguments */
 sg_host_graph *sg_host_graph_create(int model, uint64_t N, double c, uint64_t seed, uint32_t n_words);
 void sg_host_graph_destroy(sg_host_graph *g);
 /* info HOST 9 uint64: M, K (colours), dmax, entries (length of col = 2M), nslices, N, nJ (coupling entries), cap, gauge (1/0) */

@@ -22,6 +22,8 @@
  *   - energy and correlations are the observables
  *   - model 2 (RRBG): the same Hamiltonian on a bipartite random regular graph of
  *     degree 4, the paper's own ensemble
+ *   - model 3 (RRG): ... on a random regular graph of degree 4, not bipartite: the
+ *     ensemble of the main text, which Fig. S3 shows to be equivalent
  *
  * Representation: spins are UNPACKED +-1 int8, one per (site, lane), in the
  * original site labels; every lane is updated on its own with explicit
@@ -56,6 +58,7 @@
 #define OR_VB 0
 #define OR_SK 1
 #define OR_RRBG 2   /* VB Hamiltonian on a random regular bipartite graph of degree 4 */
+#define OR_RRG 3    /* ... on a random regular graph of degree 4, not bipartite (Fig. S3) */
 #define OR_MAX_SLOTS 64
 
 typedef struct or_sim {
@@ -236,7 +239,8 @@ or_sim *or_create_opt(int model, uint64_t N, double c, double T, uint64_t seed, 
                       uint32_t word0, uint32_t clones, int aligned)
 {
     if (N < 2 || N >= (1ull << 32) || n_words == 0) return NULL;
-    if (model != OR_VB && model != OR_SK && model != OR_RRBG) return NULL;
+    if (model != OR_VB && model != OR_SK && model != OR_RRBG && model != OR_RRG) return NULL;
+    if (model == OR_RRG && (N < 8 || N >= (1ull << 30))) return NULL;
     if (model == OR_RRBG && (N < 8 || (N & 1))) return NULL;   /* two halves of N/2 >= 4 vertices */
     if (!(T >= 0.0)) return NULL;
     if (clones < 1 || clones > 2 || (clones > 1 && model != OR_SK)) return NULL;
@@ -285,6 +289,52 @@ or_sim *or_create_opt(int model, uint64_t N, double c, double T, uint64_t seed, 
         h->model = OR_VB;   /* from here on: the VB Hamiltonian (Eq. 3) on this edge list */
         if (build_csr_colour_thr(h)) { or_destroy(h); return NULL; }
         const uint64_t M = h->M;
+        h->kappa = (uint64_t *)malloc((M * h->W + 1) * sizeof(uint64_t));
+        for (uint64_t f = 0; f < M; ++f)
+            for (uint32_t w = 0; w < h->W; ++w) {
+                uint32_t x[4];
+                P(h, (uint32_t)f, h->word0 + w, 0, 2, x);
+                h->kappa[f * h->W + w] = (uint64_t)x[0] | ((uint64_t)x[1] << 32);
+            }
+    } else if (model == OR_RRG) {
+        /* O2c (Q27): random regular graph of degree 4 ("random regular graphs with fixed degree
+         * z = 4"; :262 Fig. S3 compares it with the bipartite one) by the pairing model: 4N points, point q belongs to
+         * vertex q / 4; attempt t = 0, 1, 2, ... is a Fisher-Yates shuffle of the points, for i = 4N-1 down to 1:
+         * j = (x * (i+1)) >> 32 with x = word n&3 of P(n>>2, t, 0, tag 5), n = 4N-1-i, swap(p[i], p[j]); the shuffled
+         * points are paired (p[2k], p[2k+1]), k < 2N; the first attempt without a loop and without a repeated pair is
+         * the graph (uniform over simple 4-regular graphs); edge k joins p[2k]/4 and p[2k+1]/4. */
+        const uint64_t Q = 4 * N, M = 2 * N;
+        h->M = M;
+        h->eu = (uint32_t *)malloc((M + 1) * sizeof(uint32_t));
+        h->ev = (uint32_t *)malloc((M + 1) * sizeof(uint32_t));
+        uint32_t *pt = (uint32_t *)malloc(Q * sizeof(uint32_t));
+        uint32_t *nbr = (uint32_t *)malloc(Q * sizeof(uint32_t));   /* up to 4 neighbours per vertex */
+        uint8_t *cnt = (uint8_t *)malloc(N);
+        for (uint64_t t = 0;; ++t) {
+            for (uint64_t q = 0; q < Q; ++q) pt[q] = (uint32_t)q;
+            uint32_t x[4] = {0, 0, 0, 0};
+            for (uint64_t i = Q - 1; i >= 1; --i) {
+                const uint64_t n = Q - 1 - i;
+                if ((n & 3) == 0) P(h, (uint32_t)(n >> 2), (uint32_t)t, 0, 5, x);
+                const uint64_t j = ((uint64_t)x[n & 3] * (i + 1)) >> 32;
+                const uint32_t tmp = pt[i]; pt[i] = pt[j]; pt[j] = tmp;
+            }
+            memset(cnt, 0, N);
+            int simple = 1;
+            for (uint64_t k = 0; k < M && simple; ++k) {
+                const uint32_t u = pt[2 * k] / 4, v = pt[2 * k + 1] / 4;
+                if (u == v) { simple = 0; break; }
+                for (uint32_t a = 0; a < cnt[u]; ++a)
+                    if (nbr[4ull * u + a] == v) { simple = 0; break; }
+                nbr[4ull * u + cnt[u]++] = v;
+                nbr[4ull * v + cnt[v]++] = u;
+                h->eu[k] = u; h->ev[k] = v;
+            }
+            if (simple) break;
+        }
+        free(pt); free(nbr); free(cnt);
+        h->model = OR_VB;   /* from here on: the VB Hamiltonian (Eq. 3) on this edge list */
+        if (build_csr_colour_thr(h)) { or_destroy(h); return NULL; }
         h->kappa = (uint64_t *)malloc((M * h->W + 1) * sizeof(uint64_t));
         for (uint64_t f = 0; f < M; ++f)
             for (uint32_t w = 0; w < h->W; ++w) {

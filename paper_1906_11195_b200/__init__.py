@@ -5,6 +5,7 @@ arguments only: every step of the path runs in the library's CUDA kernels.
 """
 from .binding import (  # noqa: F401
     SG_MODEL_RRBG,
+    SG_MODEL_RRG,
     SG_MODEL_SK,
     SG_MODEL_VB,
     SGError,

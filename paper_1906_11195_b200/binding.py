@@ -9,7 +9,7 @@ import os
 
 import numpy as np
 
-SG_MODEL_VB, SG_MODEL_SK, SG_MODEL_RRBG = 0, 1, 2
+SG_MODEL_VB, SG_MODEL_SK, SG_MODEL_RRBG, SG_MODEL_RRG = 0, 1, 2, 3
 SG_OK, SG_EINVAL, SG_ENOMEM, SG_ECUDA, SG_ESLOT = 0, -1, -2, -3, -4
 SG_MAX_SLOTS = 64
 

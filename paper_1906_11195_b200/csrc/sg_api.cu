@@ -107,7 +107,7 @@ extern "C" sg_sim *sg_create_opt(int model, uint64_t N, double c, double T, uint
     if (o.reserved != 0 || o.aligned_start > 1) { sg_set_error("sg_create_opt: bad options"); return nullptr; }
     if (o.n_clones > 2 || (o.n_clones == 2 && model != SG_MODEL_SK)) { sg_set_error("sg_create_opt: n_clones must be 1, or 2 for the SK model"); return nullptr; }
     if (o.word0 % 4 != 0 || (uint64_t)o.word0 + n_words > (1u << 20)) { sg_set_error("sg_create_opt: word0 must be a multiple of 4 and word0 + n_words <= 2^20"); return nullptr; }
-    if (model != SG_MODEL_VB && model != SG_MODEL_SK && model != SG_MODEL_RRBG) { sg_set_error("sg_create: unknown model"); return nullptr; }
+    if (model != SG_MODEL_VB && model != SG_MODEL_SK && model != SG_MODEL_RRBG && model != SG_MODEL_RRG) { sg_set_error("sg_create: unknown model"); return nullptr; }
     if (N < 2 || N >= (1ull << 31) - 2) { sg_set_error("sg_create: N must satisfy 2 <= N < 2^31 - 2"); return nullptr; }
     if (n_words == 0 || n_words > 65535) { sg_set_error("sg_create: n_words must satisfy 1 <= n_words <= 65535"); return nullptr; }
     if (!(T >= 0.0)) { sg_set_error("sg_create: T must be >= 0 (T = inf allowed)"); return nullptr; }
@@ -116,9 +116,9 @@ extern "C" sg_sim *sg_create_opt(int model, uint64_t N, double c, double T, uint
     if (!sgx_device_ok(&why)) { sg_set_error("sg_create: " + why); return nullptr; }
     sg_sim *h = new (std::nothrow) sg_sim();
     if (!h) { sg_set_error("sg_create: out of host memory"); return nullptr; }
-    // RRBG is the VB Hamiltonian on another graph ensemble: only the host generator tells them apart
+    // RRBG and RRG are the VB Hamiltonian on other graph ensembles: only the host generator tells them apart
     h->graph_model = model;
-    if (model == SG_MODEL_RRBG) model = SG_MODEL_VB;
+    if (model == SG_MODEL_RRBG || model == SG_MODEL_RRG) model = SG_MODEL_VB;
     h->model = model; h->N = N; h->W = n_words; h->c = c; h->T = T; h->seed = seed;
     h->word0 = o.word0; h->clones = o.n_clones; h->aligned = o.aligned_start != 0;
     h->lanes = 64ull * n_words * o.n_clones;

@@ -128,6 +128,42 @@ static bool build_rrbg_edges(uint64_t N, uint64_t seed, VBHostGraph &g)
     return true;
 }
 
+// O2c: random regular graph of degree 4, not bipartite, by the pairing model (O2c): the
+// 4N half-edges ("points", point q on vertex q/4) are shuffled -- candidate t applies, to the identity, the swaps
+//   position 4N-1-n  <->  position (x_n * (4N-n)) >> 32,   n = 0 .. 4N-2,   x_n = word n&3 of P(n>>2, t, 0, tag 5)
+// -- and read off in consecutive pairs; the first candidate that is a simple graph is taken.  Edge k joins the vertices of
+// the points at positions 2k and 2k+1.
+static bool build_rrg_edges(uint64_t N, uint64_t seed, VBHostGraph &g)
+{
+    if (N < 8 || N >= (1ull << 30)) { sg_set_error("sg_create: the RRG model needs 8 <= N < 2^30"); return false; }
+    const uint64_t Q = 4 * N, M = 2 * N;
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    g.N = N; g.M = M;
+    g.eu.resize(M); g.ev.resize(M);
+    std::vector<uint32_t> point(Q);
+    std::vector<uint64_t> keys(M);
+    for (uint64_t t = 0;; ++t) {
+        std::iota(point.begin(), point.end(), 0u);
+        for (uint64_t n0 = 0; n0 + 1 < Q; n0 += 4) {
+            const Philox4 blk = sg_philox_host((uint32_t)(n0 >> 2), (uint32_t)t, 0u, 5u << 24, k0, k1);
+            for (uint64_t n = n0; n < std::min<uint64_t>(n0 + 4, Q - 1); ++n)
+                std::swap(point[Q - 1 - n], point[((uint64_t)blk.x[n - n0] * (Q - n)) >> 32]);
+        }
+        // simple <=> no pair inside one vertex and no two pairs on the same two vertices: sort the pair keys
+        bool simple = true;
+        for (uint64_t k = 0; k < M && simple; ++k) {
+            const uint32_t u = point[2 * k] >> 2, v = point[2 * k + 1] >> 2;
+            simple = u != v;
+            keys[k] = u < v ? ((uint64_t)u << 32 | v) : ((uint64_t)v << 32 | u);
+        }
+        if (!simple) continue;
+        std::sort(keys.begin(), keys.end());
+        if (std::adjacent_find(keys.begin(), keys.end()) != keys.end()) continue;
+        for (uint64_t k = 0; k < M; ++k) { g.eu[k] = point[2 * k] >> 2; g.ev[k] = point[2 * k + 1] >> 2; }
+        return true;
+    }
+}
+
 // O2: Erdos-Renyi G(N, M), M = floor(c N / 2 + 0.5), self-loops and repeated pairs rejected
 static bool build_er_edges(uint64_t N, double c, uint64_t seed, VBHostGraph &g)
 {
@@ -156,7 +192,8 @@ static bool build_er_edges(uint64_t N, double c, uint64_t seed, VBHostGraph &g)
 
 bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t n_words, VBHostGraph &g)
 {
-    if (model == SG_MODEL_RRBG ? !build_rrbg_edges(N, seed, g) : !build_er_edges(N, c, seed, g)) return false;
+    if (model == SG_MODEL_RRBG ? !build_rrbg_edges(N, seed, g) : model == SG_MODEL_RRG ? !build_rrg_edges(N, seed, g) : !build_er_edges(N, c, seed, g))
+        return false;
     const uint64_t M = g.M;
     // CSR in original labels, rows in increasing edge id
     g.row_ptr.assign(N + 1, 0);
@@ -312,7 +349,7 @@ extern "C" void sg_host_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c
 
 extern "C" sg_host_graph *sg_host_graph_create(int model, uint64_t N, double c, uint64_t seed, uint32_t n_words)
 {
-    if (model != SG_MODEL_VB && model != SG_MODEL_RRBG) { sg_set_error("sg_host_graph_create: graph model required"); return nullptr; }
+    if (model != SG_MODEL_VB && model != SG_MODEL_RRBG && model != SG_MODEL_RRG) { sg_set_error("sg_host_graph_create: graph model required"); return nullptr; }
     if (N < 2 || N >= (1ull << 31) - 2) { sg_set_error("sg_host_graph_create: N must satisfy 2 <= N < 2^31 - 2"); return nullptr; }
     if (n_words == 0) { sg_set_error("sg_host_graph_create: n_words must be >= 1"); return nullptr; }
     sg_host_graph *h = new sg_host_graph();

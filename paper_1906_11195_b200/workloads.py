@@ -9,7 +9,7 @@ from __future__ import annotations
 
 from dataclasses import dataclass
 
-VB, SK, RRBG = 0, 1, 2
+VB, SK, RRBG, RRG = 0, 1, 2, 3
 
 
 @dataclass(frozen=True)

@@ -46,7 +46,7 @@ def test_no_cpu_fallback(sg):
 def test_bad_arguments_are_rejected_before_touching_the_gpu(sg):
     for args in [(7, 100, 4.0, 1.0, 1, 1), (0, 1, 4.0, 1.0, 1, 1), (0, 100, 4.0, 1.0, 1, 0),
                  (0, 100, 4.0, -0.5, 1, 1), (0, 100, 4.0, float("nan"), 1, 1), (1, 40000, 0.0, 1.0, 1, 1),
-                 (0, (1 << 31) - 2, 4.0, 1.0, 1, 1), (2, 1001, 0.0, 1.0, 1, 1), (2, 6, 0.0, 1.0, 1, 1)]:
+                 (0, (1 << 31) - 2, 4.0, 1.0, 1, 1), (2, 1001, 0.0, 1.0, 1, 1), (2, 6, 0.0, 1.0, 1, 1), (3, 6, 0.0, 1.0, 1, 1), (4, 100, 4.0, 1.0, 1, 1)]:
         with pytest.raises(sg.SGError):
             sg.Sim(*args)
 
@@ -115,9 +115,10 @@ def _decode_rows(g):
 
 
 @pytest.mark.parametrize("model,N,c,seed,W", [(0, 1024, 4.0, 1, 1), (0, 5000, 4.0, 77, 4), (0, 333, 2.5, 3, 1), (0, 64, 7.0, 5, 2), (0, 100, 0.0, 1, 1),
-                                              (0, 3000, 14.0, 9, 1), (2, 8, 0.0, 1, 1), (2, 1024, 0.0, 2, 1), (2, 4102, 0.0, 3, 16)])
+                                              (0, 3000, 14.0, 9, 1), (2, 8, 0.0, 1, 1), (2, 1024, 0.0, 2, 1), (2, 4102, 0.0, 3, 16), (3, 8, 0.0, 4, 1), (3, 2500, 0.0, 5, 2)])
 def test_host_generator_matches_oracle_and_layout_is_consistent(sg, oracle_mod, model, N, c, seed, W):
-    """model 0: Erdos-Renyi (O2); model 2: random regular bipartite graph of degree 4 (O2b).  The layout rules of
+    """model 0: Erdos-Renyi (O2); model 2: random regular bipartite graph of degree 4 (O2b); model 3: random regular graph
+    of degree 4 (O2c).  The layout rules of
     include/sg.h (sg_host_graph_*) are re-derived here in plain Python from the oracle's edge list and colouring."""
     from paper_1906_11195_b200 import binding
 
