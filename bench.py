@@ -44,6 +44,9 @@ def parse():
     ap.add_argument("--windowed", type=int, default=0, metavar="S",
                     help="also time the windowed protocol: sg_sweep(1) + one sg_corr_accumulate against S stored configurations per sweep")
     ap.add_argument("--clones", type=int, default=1, help="SK: replicas that share the couplings (PAPER.md:233)")
+    ap.add_argument("--shard", default="sample", choices=["sample", "site"],
+                    help="N > 1: 'sample' = independent replicas per rank (default, no collective); 'site' = ONE instance, every "
+                         "colour class split over the ranks with an exchange of the updated slices after each class (PAPER.md:322-324)")
     ap.add_argument("--log2n", type=int, default=24)
     ap.add_argument("--n-words", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -166,8 +169,13 @@ def run_ours(args):
     from paper_1906_11195_b200.workloads import Workload, shard
 
     model = {"vb": sg.SG_MODEL_VB, "sk": sg.SG_MODEL_SK, "rrbg": sg.SG_MODEL_RRBG, "rrg": sg.SG_MODEL_RRG}[args.model]
-    wl = shard(Workload("bench", model, N, 4.0, args.T, 1, W, 0), rank, world)
+    site = args.shard == "site" and world > 1
+    wl = Workload("bench", model, N, 4.0, args.T, 1, W, 0) if site else shard(Workload("bench", model, N, 4.0, args.T, 1, W, 0), rank, world)
     sim = sg.Sim(wl.model, wl.N, wl.c, wl.T, wl.seed, wl.n_words, n_clones=args.clones)
+    if site:
+        from paper_1906_11195_b200.workloads import exchange_on_device, sweep_site_sharded
+
+        exch = exchange_on_device(sim, dist, rank)
     create_s = time.perf_counter() - t0
     counts = np.zeros(sim.lanes, dtype=np.uint64)
     energy = np.zeros(sim.lanes, dtype=np.int64)
@@ -176,7 +184,10 @@ def run_ours(args):
     def step(timed):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        sim.sweep(SWEEPS_PER_STEP)
+        if site:
+            sweep_site_sharded(sim, SWEEPS_PER_STEP, rank, world, exch)
+        else:
+            sim.sweep(SWEEPS_PER_STEP)
         e1.record()
         sim.snapshot(0)
         sim.correlation(0, counts)
@@ -212,7 +223,7 @@ def run_ours(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms, sweep_ms = float(t[0]), float(t[1])
     updates_per_rank = N * sim.lanes * SWEEPS_PER_STEP * args.steps
-    value = updates_per_rank * world / (ms * 1e-3)
+    value = updates_per_rank * (1 if site else world) / (ms * 1e-3)      # site-sharded: one instance, strong scaling
 
     # ---- e2e: the same step through the C-ABI with HOST buffers: the configuration goes in from pinned host
     # memory (sg_set_spins) and comes back (sg_get_spins) every step, as in the paper's flow
@@ -234,7 +245,7 @@ def run_ours(args):
             t = torch.tensor([dt], device="cuda", dtype=torch.float64)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             dt = float(t[0])
-        e2e = {"value": updates_per_rank * world / dt, "unit": "spin updates/s",
+        e2e = {"value": updates_per_rank * (1 if site else world) / dt, "unit": "spin updates/s",
                "h2d_bytes_per_step": N * sim.groups * 8, "d2h_bytes_per_step": N * sim.groups * 8 + 2 * sim.lanes * 8,
                "note": "sg_set_spins(pinned host) + step + sg_get_spins(pinned host) per step, wall clock"}
     windowed = None
@@ -279,14 +290,15 @@ def run_ours(args):
     achieved = BYTES_PER_SITE_WORD * site_words / (sweep_ms * 1e-3) / 1e9
     out = {
         "metric": METRIC, "value": value, "unit": "spin updates/s", "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if site else "weak",
         "vs_baseline": None, "dtype": "u64", "data": "synthetic",
         "config": {"workload": (f"VB N=2^{args.log2n} c=4 W={W} T={args.T} seed=1+rank (BASELINE.json configs[2])" if args.model == "vb"
                                 else f"{args.model.upper()} degree 4 N=2^{args.log2n} W={W} T={args.T} seed=1+rank (the paper's ensemble, PAPER.md:75, :260; not the headline workload)" if args.model in ("rrbg", "rrg")
                                 else f"SK N=2^{args.log2n} W={W} T={args.T} seed=1+rank (BASELINE.json configs[3]; dependency-latency bound, roofline fields not meaningful)"),
                    "step": f"sg_sweep({SWEEPS_PER_STEP}) + sg_snapshot + sg_correlation + sg_energy",
                    "l2": "inputs larger than L2: every sweep streams 777 MiB of couplings+indices+labels and reads/writes the 128 MiB spin array (L2 126 MiB); no flush needed",
-                   "parallelism": "replicas sharded by sample word, no data-path collective" if world > 1 else "single GPU",
+                   "parallelism": ("one instance sharded by site: per-class NCCL exchange of the updated slices" if site else
+                                   "replicas sharded by sample word, no data-path collective") if world > 1 else "single GPU",
                    "create_s": round(create_s, 2)},
         "roofline": {"bound": "hbm", "kernel": "k_vb_sweep (the 6-7 colour-class launches of a sweep)", "achieved": achieved, "peak": peak,
                      "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,

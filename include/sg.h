@@ -131,6 +131,33 @@ int sg_corr_configure(sg_sim *h, uint32_t nbins);
 int sg_corr_accumulate(sg_sim *h, uint32_t n, const uint32_t *slots, const uint32_t *bins);
 int sg_corr_fetch(sg_sim *h, uint32_t bin0, uint32_t nbins, uint64_t *out, uint64_t *n_out);
 
+/*
+ * Site-sharded sweeps over several GPUs ("each half of the lattice is split among the GPUs; every GPU
+ * holds a full copy of the spins; the updated spins are exchanged at each iteration, overlapped with the update").  VB
+ * models only.  A colour class is a sequence of units (the slices of the device layout); every rank holds the whole
+ * instance, updates its own units of the class, and the ranks exchange the spin words those units own before the next
+ * class starts.  The library provides the pieces; the exchange itself is a collective of the caller
+ * (paper_1906_11195_b200.workloads.sweep_site_sharded drives torch.distributed with them):
+ *   sg_class_units       number of units of colour class k.
+ *   sg_sweep_part        update units unit0 .. unit0+n-1 of class k at the current sweep index.  Asynchronous; the sweep
+ *                        counter does not move.  Updating every unit of every class in class order, then sg_end_sweep, is
+ *                        exactly sg_sweep(1).
+ *   sg_end_sweep         sweep counter += 1.
+ *   sg_part_range        the contiguous range [first, first + count) of 64-bit words of the device spin array that those
+ *                        units own (device order: position-major, word-minor, gauge-transformed -- identical on every
+ *                        rank because the layout is a function of (model, N, c, seed, n_words) only).
+ *   sg_spin_device_pointer  the ONE device pointer that crosses this interface: the spin array (sg_num_sites()*n_words
+ *                        uint64), so that a device-to-device collective (NCCL over NVLink) can exchange the ranges in
+ *                        place.  sg_export_part / sg_import_part do the same through HOST buffers.
+ */
+int sg_class_units(sg_sim *h, uint32_t k, uint64_t *n_units);
+int sg_sweep_part(sg_sim *h, uint32_t k, uint64_t unit0, uint64_t n_units);
+int sg_end_sweep(sg_sim *h);
+int sg_part_range(sg_sim *h, uint32_t k, uint64_t unit0, uint64_t n_units, uint64_t *first_word, uint64_t *n_words);
+int sg_spin_device_pointer(sg_sim *h, void **ptr);
+int sg_export_part(sg_sim *h, uint64_t first_word, uint64_t n_words, uint64_t *out /* HOST */);
+int sg_import_part(sg_sim *h, uint64_t first_word, uint64_t n_words, const uint64_t *in /* HOST */);
+
 /* Message of the last failure on this thread ("" if none). */
 const char *sg_last_error(void);
 

@@ -49,6 +49,7 @@ def lib() -> C.CDLL:
         L.or_destroy.restype = None
         L.or_sweep.argtypes = [vp, u64]
         L.or_sk_update_range.argtypes = [vp, u64, u64]
+        L.or_vb_update_sites.argtypes = [vp, vp, u64]
         L.or_snapshot.argtypes = [vp, u32]
         L.or_correlation.argtypes = [vp, u32, vp]
         L.or_energy.argtypes = [vp, vp]
@@ -125,6 +126,11 @@ class Oracle:
     # --- the five calls
     def sweep(self, n: int = 1):
         rc = self._L.or_sweep(self._h, n)
+        assert rc == 0
+
+    def vb_update_sites(self, sites):
+        sites = np.ascontiguousarray(np.asarray(sites, dtype=np.uint32))
+        rc = self._L.or_vb_update_sites(self._h, _p(sites), sites.size)
         assert rc == 0
 
     def sk_update_range(self, i0: int, i1: int):

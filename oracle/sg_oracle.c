@@ -514,6 +514,19 @@ int or_sweep(or_sim *h, uint64_t n)
     return 0;
 }
 
+/* VB only: the Metropolis update of the listed sites, in the listed order, at the current sweep index; the sweep
+ * counter does not move.  A sweep is the composition of its site updates in colour-class order (O7), so a test can
+ * let several ranks each update a part of a class and exchange the results. */
+int or_vb_update_sites(or_sim *h, const uint32_t *sites, uint64_t n)
+{
+    if (!h || h->model != OR_VB) return -1;
+    for (uint64_t q = 0; q < n; ++q) {
+        if (sites[q] >= h->N) return -1;
+        vb_update_site(h, sites[q], h->sweep);
+    }
+    return 0;
+}
+
 /* SK only: the updates of sites i0 .. i1-1 of the sweep with the current index, in order, on the current
  * configuration; the sweep counter does not move.  A sweep is the composition of its N site updates ("N
  * single spin updates, performed in a fixed order"), so tests can check a window of a very large instance: sites

@@ -30,6 +30,13 @@ SYMBOLS = {
     "sg_corr_configure": (C.c_int, [_vp, _u32]),
     "sg_corr_accumulate": (C.c_int, [_vp, _u32, _vp, _vp]),
     "sg_corr_fetch": (C.c_int, [_vp, _u32, _u32, _vp, _vp]),
+    "sg_class_units": (C.c_int, [_vp, _u32, _vp]),
+    "sg_sweep_part": (C.c_int, [_vp, _u32, _u64, _u64]),
+    "sg_end_sweep": (C.c_int, [_vp]),
+    "sg_part_range": (C.c_int, [_vp, _u32, _u64, _u64, _vp, _vp]),
+    "sg_spin_device_pointer": (C.c_int, [_vp, _vp]),
+    "sg_export_part": (C.c_int, [_vp, _u64, _u64, _vp]),
+    "sg_import_part": (C.c_int, [_vp, _u64, _u64, _vp]),
     "sg_last_error": (C.c_char_p, []),
     "sg_sweep_count": (_u64, [_vp]),
     "sg_num_edges": (_u64, [_vp]),
@@ -211,6 +218,49 @@ class Sim:
         hits = np.zeros(nbins, dtype=np.uint64)
         _check(self._L.sg_corr_fetch(self._h, int(bin0), int(nbins), _ptr(out), _ptr(hits)))
         return out, hits
+
+    # --- site-sharded sweeps (include/sg.h): the backend interface of workloads.sweep_site_sharded
+    def class_units(self, k: int) -> int:
+        n = C.c_uint64(0)
+        _check(self._L.sg_class_units(self._h, int(k), C.byref(n)))
+        return int(n.value)
+
+    def sweep_part(self, k: int, unit0: int, n_units: int):
+        _check(self._L.sg_sweep_part(self._h, int(k), int(unit0), int(n_units)))
+
+    def end_sweep(self):
+        _check(self._L.sg_end_sweep(self._h))
+
+    def part_range(self, k: int, unit0: int, n_units: int):
+        a, b = C.c_uint64(0), C.c_uint64(0)
+        _check(self._L.sg_part_range(self._h, int(k), int(unit0), int(n_units), C.byref(a), C.byref(b)))
+        return int(a.value), int(b.value)
+
+    def export_part(self, k: int, unit0: int, n_units: int) -> np.ndarray:
+        first, n = self.part_range(k, unit0, n_units)
+        out = np.zeros(n, dtype=np.uint64)
+        _check(self._L.sg_export_part(self._h, first, n, _ptr(out)))
+        return out
+
+    def import_part(self, k: int, unit0: int, n_units: int, words: np.ndarray):
+        first, n = self.part_range(k, unit0, n_units)
+        words = np.ascontiguousarray(words, dtype=np.uint64)
+        assert words.size == n
+        _check(self._L.sg_import_part(self._h, first, n, _ptr(words)))
+
+    def spin_tensor(self):
+        """The device spin array as a torch tensor (int64 view of the uint64 words) sharing the library's memory: for
+        device-to-device collectives on the ranges of part_range()."""
+        import torch
+
+        p = C.c_void_p(0)
+        _check(self._L.sg_spin_device_pointer(self._h, C.byref(p)))
+        n = self.N * self.W
+
+        class _Arr:
+            __cuda_array_interface__ = {"shape": (n,), "typestr": "<i8", "data": (int(p.value), False), "version": 3}
+
+        return torch.as_tensor(_Arr(), device=torch.device("cuda", torch.cuda.current_device()))
 
     @property
     def sweep_count(self) -> int:

@@ -157,6 +157,78 @@ extern "C" int sg_sweep(sg_sim *h, uint64_t n)
     return SG_OK;
 }
 
+// ---- site-sharded sweeps -----------------------------------------------------------------------------
+static bool vb_part_ok(sg_sim *h, uint32_t k, uint64_t unit0, uint64_t n, const char *who)
+{
+    if (!h || h->model != SG_MODEL_VB) { sg_set_error(std::string(who) + ": VB handle required"); return false; }
+    if (k >= h->g.K || unit0 + n > h->g.cls[k].nslices) { sg_set_error(std::string(who) + ": class or unit range out of bounds"); return false; }
+    return true;
+}
+
+extern "C" int sg_class_units(sg_sim *h, uint32_t k, uint64_t *n_units)
+{
+    if (!n_units || !vb_part_ok(h, k, 0, 0, "sg_class_units")) return SG_EINVAL;
+    *n_units = h->g.cls[k].nslices;
+    return SG_OK;
+}
+
+extern "C" int sg_sweep_part(sg_sim *h, uint32_t k, uint64_t unit0, uint64_t n_units)
+{
+    if (!vb_part_ok(h, k, unit0, n_units, "sg_sweep_part")) return SG_EINVAL;
+    if (n_units == 0) return SG_OK;
+    VBClass part = h->g.cls[k];
+    part.slice0 += unit0;
+    part.nslices = n_units;
+    part.n = 1;       // non-empty (the kernels take their positions from the slice headers)
+    return sgk_vb_sweep_class(h->vb, part, h->g.N, h->vb_nJ, h->W, h->word0, h->sweep, h->key, false, sgx_stream());
+}
+
+extern "C" int sg_end_sweep(sg_sim *h)
+{
+    if (!h || h->sweep + 1 >= (1ull << 56)) { sg_set_error("sg_end_sweep: bad handle or counter overflow"); return SG_EINVAL; }
+    h->sweep++;
+    return SG_OK;
+}
+
+extern "C" int sg_part_range(sg_sim *h, uint32_t k, uint64_t unit0, uint64_t n_units, uint64_t *first_word, uint64_t *n_words)
+{
+    if (!first_word || !n_words || !vb_part_ok(h, k, unit0, n_units, "sg_part_range")) return SG_EINVAL;
+    const uint64_t s0 = h->g.cls[k].slice0 + unit0;
+    const uint64_t p0 = h->g.hdr[s0].pos0;
+    // the next slice of the same class starts where this range ends; after the last slice of the class the class ends
+    const uint64_t p1 = unit0 + n_units < h->g.cls[k].nslices ? h->g.hdr[s0 + n_units].pos0 : h->g.cls[k].pos0 + h->g.cls[k].n;
+    *first_word = p0 * h->W;
+    *n_words = (n_units ? p1 - p0 : 0) * h->W;
+    return SG_OK;
+}
+
+extern "C" int sg_spin_device_pointer(sg_sim *h, void **ptr)
+{
+    if (!h || !ptr || h->model != SG_MODEL_VB) { sg_set_error("sg_spin_device_pointer: VB handle required"); return SG_EINVAL; }
+    *ptr = h->vb.spin;
+    return SG_OK;
+}
+
+extern "C" int sg_export_part(sg_sim *h, uint64_t first_word, uint64_t n_words, uint64_t *out)
+{
+    if (!h || h->model != SG_MODEL_VB || (n_words && !out) || first_word + n_words > h->spin_words) { sg_set_error("sg_export_part: bad argument"); return SG_EINVAL; }
+    cudaStream_t st = sgx_stream();
+    if (n_words && (!cuda_ok(cudaMemcpyAsync(out, h->vb.spin + first_word, n_words * 8, cudaMemcpyDeviceToHost, st), "sg_export_part") ||
+                    !cuda_ok(cudaStreamSynchronize(st), "sg_export_part")))
+        return SG_ECUDA;
+    return SG_OK;
+}
+
+extern "C" int sg_import_part(sg_sim *h, uint64_t first_word, uint64_t n_words, const uint64_t *in)
+{
+    if (!h || h->model != SG_MODEL_VB || (n_words && !in) || first_word + n_words > h->spin_words) { sg_set_error("sg_import_part: bad argument"); return SG_EINVAL; }
+    cudaStream_t st = sgx_stream();
+    if (n_words && (!cuda_ok(cudaMemcpyAsync(h->vb.spin + first_word, in, n_words * 8, cudaMemcpyHostToDevice, st), "sg_import_part") ||
+                    !cuda_ok(cudaStreamSynchronize(st), "sg_import_part")))
+        return SG_ECUDA;
+    return SG_OK;
+}
+
 static uint64_t *current_config(sg_sim *h) { return h->model == SG_MODEL_VB ? h->vb.spin : h->sk.spin; }
 
 extern "C" int sg_snapshot(sg_sim *h, uint32_t slot)

@@ -168,3 +168,69 @@ def run_windowed(sim, total_sweeps: int, tws=(4, 16, 64, 256, 1024, 4096), binni
         if time in slot_of:
             sim.snapshot(slot_of[time])
     return out
+
+
+# ---- site-sharded sweeps over several ranks -------------------------------------
+def split_units(n_units: int, rank: int, world: int):
+    """Units [a, b) of a class that rank `rank` of `world` updates: contiguous, balanced to within one unit."""
+    if not 0 <= rank < world:
+        raise ValueError("rank out of range")
+    return n_units * rank // world, n_units * (rank + 1) // world
+
+
+def sweep_site_sharded(backend, n_sweeps: int, rank: int, world: int, exchange):
+    """The paper's multi-GPU scheme on any backend with n_colours, class_units(k), sweep_part(k, unit0, n),
+    end_sweep() (the binding's Sim on a GPU, or tests' oracle backend): every rank holds the full configuration; for
+    each colour class in order a rank updates its own units, then `exchange(k, parts)` -- parts[r] = (unit0, n) of every
+    rank -- makes every rank's copy of the class current before the next class starts.  No arithmetic of the method
+    here.  The result on every rank equals backend.sweep(n_sweeps) on one rank, bit for bit."""
+    for _ in range(n_sweeps):
+        for k in range(backend.n_colours):
+            units = backend.class_units(k)
+            parts = []
+            for r in range(world):
+                a, b = split_units(units, r, world)
+                parts.append((a, b - a))
+            backend.sweep_part(k, *parts[rank])
+            if world > 1:
+                exchange(k, parts)
+        backend.end_sweep()
+
+
+def exchange_through_host(backend, dist, rank: int):
+    """exchange() for sweep_site_sharded with host buffers and torch.distributed broadcasts (any backend, gloo or nccl)."""
+    import numpy as np
+    import torch
+
+    def exchange(k, parts):
+        for r, (u0, n) in enumerate(parts):
+            if n == 0:
+                continue
+            if r == rank:
+                buf = torch.from_numpy(backend.export_part(k, u0, n).view(np.int64).copy())
+            else:
+                buf = torch.empty(backend.part_range(k, u0, n)[1], dtype=torch.int64)
+            dist.broadcast(buf, src=r)
+            if r != rank:
+                backend.import_part(k, u0, n, buf.numpy().view(np.uint64))
+
+    return exchange
+
+
+def exchange_on_device(sim, dist, rank: int):
+    """exchange() for the binding's Sim on GPUs: NCCL broadcasts of each rank's contiguous range of the device spin array,
+    in place (NVLink / NVSwitch), on torch's current stream -- the stream the library launches on, so the next class's
+    kernels are ordered after the exchange."""
+    spins = sim.spin_tensor()
+
+    def exchange(k, parts):
+        works = []
+        for r, (u0, n) in enumerate(parts):
+            if n == 0:
+                continue
+            first, count = sim.part_range(k, u0, n)
+            works.append(dist.broadcast(spins[first:first + count], src=r, async_op=True))
+        for w in works:
+            w.wait()
+
+    return exchange

@@ -475,3 +475,52 @@ def test_bipartition_is_statistically_irrelevant(sg):
         assert abs(a.mean() - b.mean()) < 0.02 * max(a.mean(), 0.25), (k, a.mean(), b.mean())
         means.append(a.mean())
     assert means[0] > 0.6 and means[-1] < 0.05             # C decays from 0.62 to 0.02 over t = 1 .. 1024
+
+
+def test_site_sharded_parts_compose_to_the_sweep(sg, oracle_mod):
+    """The pieces of the site-sharded multi-GPU sweep (include/sg.h) on one GPU: updating every class
+    part by part -- as three ranks would, each on its own copy, with the parts exchanged through host buffers or
+    through the device tensor -- reproduces sg_sweep bit for bit."""
+    import torch
+
+    from paper_1906_11195_b200.workloads import split_units, sweep_site_sharded
+
+    N, W, world = 20000, 2, 3
+    ref = sg.Sim(sg.SG_MODEL_VB, N, 4.0, 1.0, 23, W)
+    o = oracle_mod.Oracle(oracle_mod.VB, N, 4.0, 1.0, 23, W)
+    ranks = [sg.Sim(sg.SG_MODEL_VB, N, 4.0, 1.0, 23, W) for _ in range(world)]      # one full copy per emulated rank
+    tensors = [r.spin_tensor() for r in ranks]
+    assert all(t.numel() == N * W and t.is_cuda for t in tensors)
+    for sweep in range(3):
+        for k in range(ref.n_colours):
+            units = ref.class_units(k)
+            parts = [split_units(units, r, world) for r in range(world)]
+            for r, (a, b) in enumerate(parts):
+                ranks[r].sweep_part(k, a, b - a)
+            for r, (a, b) in enumerate(parts):                       # the exchange: every part to every other rank
+                first, count = ranks[r].part_range(k, a, b - a)
+                if sweep % 2 == 0:
+                    words = ranks[r].export_part(k, a, b - a)
+                    assert words.size == count
+                    for q in range(world):
+                        if q != r:
+                            ranks[q].import_part(k, a, b - a, words)
+                else:
+                    torch.cuda.synchronize()
+                    for q in range(world):
+                        if q != r:
+                            tensors[q][first:first + count].copy_(tensors[r][first:first + count])
+                    torch.cuda.synchronize()
+        for r in ranks:
+            r.end_sweep()
+        ref.sweep(1)
+        o.sweep(1)
+        for r in ranks:
+            assert r.sweep_count == ref.sweep_count
+            assert np.array_equal(r.spins(), ref.spins())
+        assert np.array_equal(ref.spins(), o.spins())
+    one = sg.Sim(sg.SG_MODEL_VB, N, 4.0, 1.0, 23, W)
+    sweep_site_sharded(one, 3, 0, 1, None)
+    assert np.array_equal(one.spins(), ref.spins())
+    with pytest.raises(sg.SGError):
+        one.sweep_part(0, 0, one.class_units(0) + 1)
