@@ -169,6 +169,6 @@ def test_bits_are_fair(oracle_mod):
 
 def test_create_rejects_bad_arguments(oracle_mod):
     for args in [(0, 1, 4.0, 1.0, 1, 1), (0, 100, 4.0, 1.0, 1, 0), (0, 10, 40.0, 1.0, 1, 1),
-                 (0, 100, 4.0, -1.0, 1, 1), (3, 100, 4.0, 1.0, 1, 1), (1, 40000, 0.0, 1.0, 1, 1)]:
+                 (0, 100, 4.0, -1.0, 1, 1), (4, 100, 4.0, 1.0, 1, 1), (1, 40000, 0.0, 1.0, 1, 1)]:
         with pytest.raises(ValueError):
             oracle_mod.Oracle(*args)
