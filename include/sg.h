@@ -215,32 +215,36 @@ void sg_host_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t
  * Gauge: the BFS forest's edges ("tree entries", T) carry no coupling word: with eps_root = 0 and
  * eps_child = eps_parent ^ kappa_(tree edge) the device stores sigma ^ eps and kappa_ij ^ eps_i ^ eps_j, which leaves
  * every bond state sigma_i ^ sigma_j ^ kappa_ij, hence every output, unchanged.  The other entries ("X") keep a word.
- * Slices: every class is cut greedily, in position order, into runs of at most 32 sites whose T entries and whose X
- * entries number at most `cap` each (cap depends on n_words only).  hdr[g] = 4 uint32: first position, first index in
- * col, first coupling entry, and n | nTs << 6 | nXs << 16 (sites, T entries, X entries of the slice); one sentinel
- * follows the last slice.  col holds, slice after slice, the T entries in site order (per site: parent first, then the
- * children by ascending position), then the X entries in site order (per site by ascending position); the coupling
- * entries follow the X order, jeid gives the edge id of each.  orig_s[32g + j] = label of the j-th site of slice g
- * (0xFFFFFFFF for j >= n); rp_s[32g + j] = tOff | xOff << 10 | nT << 20 | nX << 25: where the site's entries start
- * inside the slice's T run / X run, and how many there are.  No output depends on any of this: the Philox counter
+ * Slices: every class is cut greedily, in position order, into runs of at most 32 sites with at most 32*it entries of
+ * which at most 32*itx are X entries; (it, itx) is chosen per class, from the class's degrees, among the budgets the
+ * kernels are compiled for ((4,3), (5,4), (6,4), (8,6) for odd n_words: the one that minimises
+ * slices * (200 + 13 it); (4,3) for n_words = 2 mod 4; (4,2) for n_words = 0 mod 4).  hdr[g] = 4 uint32: first
+ * position, first index in col, first coupling entry, and n | nXs << 6 | nE << 16 (sites, X entries, all entries of the
+ * slice); one sentinel follows the last slice.  col holds, slice after slice, ONE run of nE neighbour positions: the
+ * X entries in site order (per site by ascending position), then the T entries in site order (per site: parent first,
+ * then the children by ascending position); the coupling entries follow the X order, jeid gives the edge id of each.
+ * orig_s[32g + j] = label of the j-th site of slice g (0xFFFFFFFF for j >= n); rp_s[32g + j] =
+ * xOff | tOff << 8 | nX << 16 | nT << 21: where the site's X / T entries start inside the slice's run (tOff >= nXs),
+ * and how many there are.  No output depends on any of this: the Philox counter
  * uses the original label (Q15).
  */
 typedef struct sg_host_graph sg_host_graph;
 /* model: SG_MODEL_VB, SG_MODEL_RRBG or SG_MODEL_RRG; NULL on bad arguments */
 sg_host_graph *sg_host_graph_create(int model, uint64_t N, double c, uint64_t seed, uint32_t n_words);
 void sg_host_graph_destroy(sg_host_graph *g);
-/* info HOST 9 uint64: M, K (colours), dmax, entries (length of col = 2M), nslices, N, nJ (coupling entries), cap, gauge (1/0) */
+/* info HOST 9 uint64: M, K (colours), dmax, entries (length of col = 2M), nslices, N, nJ (coupling entries), it_max (largest per-class it), gauge (1/0) */
 int sg_host_graph_info(const sg_host_graph *g, uint64_t *info);
 /*
  * Copies out whichever arrays are non-NULL (all HOST): u,v M uint32; colour N uint32; orig N uint32
  * (position -> label); hdr 4*(nslices+1) uint32; orig_s, rp_s 32*nslices uint32; col entries uint32; jeid nJ uint32;
  * tpar, teid N uint32 (parent position / tree edge id, 0xFFFFFFFF for roots); bfs_pos N uint32 (positions in
- * breadth-first order); class_pos0, class_n, class_slice0, class_nslices K uint64 each.
+ * breadth-first order); class_pos0, class_n, class_slice0, class_nslices, class_it, class_itx K uint64 each.
  */
 int sg_host_graph_get(const sg_host_graph *g, uint32_t *u, uint32_t *v, uint32_t *colour, uint32_t *orig,
                       uint32_t *hdr, uint32_t *orig_s, uint32_t *rp_s, uint32_t *col, uint32_t *jeid,
                       uint32_t *tpar, uint32_t *teid, uint32_t *bfs_pos,
-                      uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0, uint64_t *class_nslices);
+                      uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0, uint64_t *class_nslices,
+                      uint64_t *class_it, uint64_t *class_itx);
 
 /*
  * Number of kernels this library has launched (process-wide, all handles) since load.

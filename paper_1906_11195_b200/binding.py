@@ -54,7 +54,7 @@ SYMBOLS = {
     "sg_host_graph_create": (_vp, [C.c_int, _u64, _dbl, _u64, _u32]),
     "sg_host_graph_destroy": (None, [_vp]),
     "sg_host_graph_info": (C.c_int, [_vp, _vp]),
-    "sg_host_graph_get": (C.c_int, [_vp] * 17),
+    "sg_host_graph_get": (C.c_int, [_vp] * 19),
 }
 
 
@@ -332,18 +332,18 @@ def host_graph(N: int, c: float, seed: int, model: int = SG_MODEL_VB, n_words: i
     try:
         info = np.zeros(9, dtype=np.uint64)
         _check(L.sg_host_graph_info(g, _ptr(info)))
-        M, K, dmax, entries, nslices, N, nJ, cap, gauge = (int(x) for x in info)
-        a = dict(M=M, K=K, dmax=dmax, entries=entries, nslices=nslices, N=N, nJ=nJ, cap=cap, gauge=gauge)
+        M, K, dmax, entries, nslices, N, nJ, it_max, gauge = (int(x) for x in info)
+        a = dict(M=M, K=K, dmax=dmax, entries=entries, nslices=nslices, N=N, nJ=nJ, it_max=it_max, gauge=gauge)
         a["u"] = np.zeros(M, np.uint32); a["v"] = np.zeros(M, np.uint32)
         for k in ("colour", "orig", "tpar", "teid", "bfs_pos"):
             a[k] = np.zeros(N, np.uint32)
         a["hdr"] = np.zeros((nslices + 1, 4), np.uint32)
         a["orig_s"] = np.zeros(32 * nslices, np.uint32); a["rp_s"] = np.zeros(32 * nslices, np.uint32)
         a["col"] = np.zeros(entries, np.uint32); a["jeid"] = np.zeros(nJ, np.uint32)
-        for k in ("class_pos0", "class_n", "class_slice0", "class_nslices"):
+        for k in ("class_pos0", "class_n", "class_slice0", "class_nslices", "class_it", "class_itx"):
             a[k] = np.zeros(K, np.uint64)
         _check(L.sg_host_graph_get(g, *(_ptr(a[k]) for k in ("u", "v", "colour", "orig", "hdr", "orig_s", "rp_s", "col", "jeid", "tpar",
-                                                              "teid", "bfs_pos", "class_pos0", "class_n", "class_slice0", "class_nslices"))))
+                                                              "teid", "bfs_pos", "class_pos0", "class_n", "class_slice0", "class_nslices", "class_it", "class_itx"))))
         return a
     finally:
         L.sg_host_graph_destroy(g)

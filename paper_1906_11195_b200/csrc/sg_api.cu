@@ -48,7 +48,7 @@ int create_vb(sg_sim *h)
     h->spin_words = N * W;
     h->vb_nJ = nJ;
     h->vb.nslices = (uint32_t)nslices;
-    h->vb.cap = g.cap;
+    h->vb.it_max = g.it_max; h->vb.itx_max = g.itx_max;
     h->vb.spin = dev_alloc<uint64_t>(h, N * W);
     h->vb.eps = dev_alloc<uint64_t>(h, N * W);
     h->vb.J = dev_alloc<uint64_t>(h, nJ * W + 4);
@@ -437,12 +437,12 @@ extern "C" int sg_get_couplings(sg_sim *h, uint64_t *out)
     };
     for (uint64_t s = 0; s < nslices; ++s) {
         const SGHdr &hd = g.hdr[s];
-        const uint32_t n = hd.counts & 63u, nTs = (hd.counts >> 6) & 1023u;
+        const uint32_t n = hd.counts & 63u;
         for (uint32_t j = 0; j < n; ++j) {
-            const uint32_t rp = g.rp_s[32 * s + j], xOff = (rp >> 10) & 1023u, nX = rp >> 25;
+            const uint32_t rp = g.rp_s[32 * s + j], xOff = rp & 255u, nX = (rp >> 16) & 31u;
             const uint64_t p = (uint64_t)hd.pos0 + j;
             for (uint32_t r = 0; r < nX; ++r) {
-                const uint64_t nb = col[(uint64_t)hd.col_off + nTs + xOff + r], x = (uint64_t)hd.j_off + xOff + r;
+                const uint64_t nb = col[(uint64_t)hd.col_off + xOff + r], x = (uint64_t)hd.j_off + xOff + r;
                 const uint32_t e = edge_between(g.orig[p], g.orig[nb]);
                 if (e == SG_NONE) { sg_set_error("sg_get_couplings: a stored entry is not an edge of the graph"); return SG_ECUDA; }
                 for (uint32_t w = 0; w < W; ++w) {

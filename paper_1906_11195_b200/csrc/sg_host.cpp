@@ -252,15 +252,15 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t 
     const bool label_order = order_env && !std::strcmp(order_env, "label");
     const char *gauge_env = std::getenv("SG_VB_GAUGE");
     g.gauge = !(gauge_env && !std::strcmp(gauge_env, "0"));                 // measurement knob: keep every coupling word
-    const char *cap_env = std::getenv("SG_VB_CAP");                          // measurement knob: entry budget of a slice
-    g.cap = cap_env ? (uint32_t)std::min(1023, std::max(31, std::atoi(cap_env))) : sg_vb_slice_cap(n_words);
-
     // per site: tree entries nT (parent + children); the others are X entries
     std::vector<uint8_t> nT(N, 0);
     if (g.gauge)
         for (uint64_t i = 0; i < N; ++i)
             if (par[i] != SG_NONE) { nT[i]++; nT[par[i]]++; }
-    // positions: (class, breadth-first index)
+    auto shape_of = [&](uint32_t i) { return sg_vb_shape((uint32_t)(g.row_ptr[i + 1] - g.row_ptr[i]) - nT[i], nT[i]); };
+    const char *win_env = std::getenv("SG_VB_WIN");                         // measurement knob: 0 = no shape sort
+    const uint64_t win = win_env ? (uint64_t)std::max(0, std::atoi(win_env)) : 4096;
+    // positions: (class, window of the breadth-first index, shape, breadth-first index)
     std::vector<uint64_t> ccount(K, 0);
     for (uint64_t i = 0; i < N; ++i) ccount[g.colour[i]]++;
     g.cls.assign(K, VBClass{});
@@ -274,6 +274,22 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t 
         for (uint32_t k = 0; k < K; ++k) fill[k] = g.cls[k].pos0;
         if (label_order) for (uint64_t i = 0; i < N; ++i) g.orig[fill[g.colour[i]]++] = (uint32_t)i;
         else for (uint64_t q = 0; q < N; ++q) g.orig[fill[g.colour[bfs[q]]]++] = bfs[q];
+        // Shape buckets: every window of `win` consecutive sites of a class (in the order above) is stably sorted by
+        // the site's shape (sg_vb_shape: 0 = at most 2 X and 2 T entries, 1 = at most 4 and 4, 2 = longer rows), so
+        // that almost every slice holds sites of one shape and the kernels run the count that fits it.  The
+        // breadth-first order survives inside each of the three runs of a window.
+        if (win > 1) {
+            std::vector<uint32_t> tmp(win);
+            for (uint32_t k = 0; k < K; ++k)
+                for (uint64_t a = g.cls[k].pos0, end = a + g.cls[k].n; a < end; a += win) {
+                    const uint64_t len = std::min<uint64_t>(win, end - a);
+                    uint64_t cnt[3] = {0, 0, 0};
+                    for (uint64_t q = 0; q < len; ++q) cnt[shape_of(g.orig[a + q])]++;
+                    uint64_t at[3] = {0, cnt[0], cnt[0] + cnt[1]};
+                    for (uint64_t q = 0; q < len; ++q) tmp[at[shape_of(g.orig[a + q])]++] = g.orig[a + q];
+                    std::copy(tmp.begin(), tmp.begin() + len, g.orig.begin() + a);
+                }
+        }
         for (uint64_t p = 0; p < N; ++p) g.pos[g.orig[p]] = (uint32_t)p;
     }
     g.tpar.assign(N, SG_NONE); g.teid.assign(N, SG_NONE);
@@ -284,25 +300,61 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t 
         const uint32_t i = g.orig[p];
         if (par[i] != SG_NONE) { g.tpar[p] = g.pos[par[i]]; g.teid[p] = par_e[i]; }
     }
-    // slices: greedy runs of <= 32 positions of one class within the entry budget
+    // per-class entry budgets (sg_internal.h): among the budgets the kernels are compiled for, the one that minimises
+    // an estimate of the warp instructions per site, slices * (fixed part + per-step part * it)
+    // (SG_VB_IT=<it> forces one budget for all classes: a measurement knob; outputs are identical)
+    const char *it_env = std::getenv("SG_VB_IT");
+    auto count_slices = [&](uint32_t k, VBBudget bud) {
+        uint64_t ns = 0, p = g.cls[k].pos0;
+        const uint64_t pend = p + g.cls[k].n;
+        while (p < pend) {
+            uint32_t n = 0, sE = 0, sX = 0;
+            while (p < pend && n < 32) {
+                const uint32_t i = g.orig[p];
+                const uint32_t d = (uint32_t)(g.row_ptr[i + 1] - g.row_ptr[i]), x = d - nT[i];
+                if (n > 0 && (sE + d > 32 * bud.it || sX + x > 32 * bud.itx)) break;
+                sE += d; sX += x; ++n; ++p;
+            }
+            ++ns;
+        }
+        return ns;
+    };
+    g.it_max = g.itx_max = 0;
+    for (uint32_t k = 0; k < K; ++k) {
+        VBBudget best = n_words % 4 == 0 ? SG_VB_BUDGET_G4 : SG_VB_BUDGET_G2;
+        if (n_words % 2 != 0) {
+            double best_cost = 0;
+            bool first = true;
+            for (const VBBudget bud : SG_VB_BUDGETS_G1) {
+                if (it_env && (uint32_t)std::atoi(it_env) != bud.it) continue;
+                const double cost = (double)count_slices(k, bud) * (200.0 + 13.0 * bud.it);
+                if (first || cost < best_cost) { best = bud; best_cost = cost; first = false; }
+            }
+            if (first) best = SG_VB_BUDGETS_G1[0];
+        }
+        g.cls[k].it = best.it; g.cls[k].itx = best.itx;
+        g.it_max = std::max(g.it_max, best.it); g.itx_max = std::max(g.itx_max, best.itx);
+    }
+    // slices: greedy runs of <= 32 positions of one class within the class's budgets
     g.hdr.clear(); g.orig_s.clear(); g.rp_s.clear();
     g.col.clear(); g.col.reserve(2 * M); g.jeid.clear();
-    std::vector<uint32_t> rowT, rowX;            // the slice's X entries are appended after its T entries
+    std::vector<uint32_t> rowT, rowX;            // the slice's T entries are appended after its X entries
     std::vector<uint32_t> rowXe;
     for (uint32_t k = 0; k < K; ++k) {
         g.cls[k].slice0 = g.hdr.size();
         uint64_t p = g.cls[k].pos0;
         const uint64_t pend = p + g.cls[k].n;
+        const uint32_t capE = 32 * g.cls[k].it, capX = 32 * g.cls[k].itx;
         while (p < pend) {
             SGHdr h{(uint32_t)p, (uint32_t)g.col.size(), (uint32_t)g.jeid.size(), 0u};
-            uint32_t n = 0, sT = 0, sX = 0;
+            uint32_t n = 0, sT = 0, sX = 0, shape = 0;
             rowT.clear(); rowX.clear(); rowXe.clear();
             const size_t base = g.orig_s.size();
             g.orig_s.resize(base + 32, SG_NONE); g.rp_s.resize(base + 32, 0u);
             while (p < pend && n < 32) {
                 const uint32_t i = g.orig[p];
                 const uint32_t d = (uint32_t)(g.row_ptr[i + 1] - g.row_ptr[i]), t = nT[i], x = d - t;
-                if (n > 0 && (sT + t > g.cap || sX + x > g.cap)) break;
+                if (n > 0 && (sT + sX + d > capE || sX + x > capX)) break;
                 // tree entries: parent first, then children by position; other entries by position
                 uint64_t keyT[32], keyX[32];
                 uint32_t cT = 0, cX = 0;
@@ -316,15 +368,17 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t 
                 std::sort(keyT + ((g.gauge && par_e[i] != SG_NONE) ? 1 : 0), keyT + cT);
                 std::sort(keyX, keyX + cX);
                 g.orig_s[base + n] = i;
-                g.rp_s[base + n] = sT | sX << 10 | cT << 20 | cX << 25;
+                g.rp_s[base + n] = sX | sT << 8 | cX << 16 | cT << 21;          // tOff is made absolute below
                 for (uint32_t q = 0; q < cT; ++q) rowT.push_back((uint32_t)(keyT[q] >> 32));
                 for (uint32_t q = 0; q < cX; ++q) { rowX.push_back((uint32_t)(keyX[q] >> 32)); rowXe.push_back((uint32_t)keyX[q]); }
+                shape = std::max(shape, sg_vb_shape(cX, cT));
                 sT += cT; sX += cX; ++n; ++p;
             }
-            h.counts = n | sT << 6 | sX << 16;
+            for (uint32_t j = 0; j < n; ++j) g.rp_s[base + j] += sX << 8;       // T entries follow the slice's X entries
+            h.counts = n | sX << 6 | (sT + sX) << 16 | shape << 28;
             g.hdr.push_back(h);
-            g.col.insert(g.col.end(), rowT.begin(), rowT.end());
             g.col.insert(g.col.end(), rowX.begin(), rowX.end());
+            g.col.insert(g.col.end(), rowT.begin(), rowT.end());
             g.jeid.insert(g.jeid.end(), rowXe.begin(), rowXe.end());
             if (g.col.size() >= (1ull << 32)) { sg_set_error("sg_create: instance too large for 32-bit entry indices"); return false; }
         }
@@ -333,10 +387,6 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t 
     g.hdr.push_back(SGHdr{(uint32_t)N, (uint32_t)g.col.size(), (uint32_t)g.jeid.size(), 0u});
     return true;
 }
-
-// Entry budget of a slice: its T and X entries are parked in shared memory (8 bytes per entry and word of the group):
-// 2 KiB per warp at one word per thread, 4 KiB at two or four.
-uint32_t sg_vb_slice_cap(uint32_t n_words) { return n_words % 4 ? 128u : 64u; }
 
 // ---- host-only C entry points (include/sg.h) ------------------------------------------------------
 struct sg_host_graph { VBHostGraph g; };
@@ -364,14 +414,15 @@ extern "C" int sg_host_graph_info(const sg_host_graph *h, uint64_t *info)
     if (!h || !info) return SG_EINVAL;
     const VBHostGraph &g = h->g;
     info[0] = g.M; info[1] = g.K; info[2] = g.dmax; info[3] = g.col.size();
-    info[4] = g.hdr.size() - 1; info[5] = g.N; info[6] = g.jeid.size(); info[7] = g.cap; info[8] = g.gauge ? 1 : 0;
+    info[4] = g.hdr.size() - 1; info[5] = g.N; info[6] = g.jeid.size(); info[7] = g.it_max; info[8] = g.gauge ? 1 : 0;
     return SG_OK;
 }
 
 extern "C" int sg_host_graph_get(const sg_host_graph *h, uint32_t *u, uint32_t *v, uint32_t *colour, uint32_t *orig,
                                  uint32_t *hdr, uint32_t *orig_s, uint32_t *rp_s, uint32_t *col, uint32_t *jeid,
                                  uint32_t *tpar, uint32_t *teid, uint32_t *bfs_pos,
-                                 uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0, uint64_t *class_nslices)
+                                 uint64_t *class_pos0, uint64_t *class_n, uint64_t *class_slice0, uint64_t *class_nslices,
+                                 uint64_t *class_it, uint64_t *class_itx)
 {
     if (!h) return SG_EINVAL;
     const VBHostGraph &g = h->g;
@@ -392,6 +443,8 @@ extern "C" int sg_host_graph_get(const sg_host_graph *h, uint32_t *u, uint32_t *
         if (class_n) class_n[k] = g.cls[k].n;
         if (class_slice0) class_slice0[k] = g.cls[k].slice0;
         if (class_nslices) class_nslices[k] = g.cls[k].nslices;
+        if (class_it) class_it[k] = g.cls[k].it;
+        if (class_itx) class_itx[k] = g.cls[k].itx;
     }
     return SG_OK;
 }

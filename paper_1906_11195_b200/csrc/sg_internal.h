@@ -29,17 +29,22 @@ Philox4 sg_philox_host(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint3
 // s_i -> eps_i s_i, J_ij -> eps_i J_ij eps_j with eps_child = eps_parent * J_(parent,child) (eps_root = +1), which
 // changes no bond state, hence no flip decision, energy or correlation count.  The device stores the
 // transformed spins and couplings; tree entries ("T") need no coupling word at all, the others ("X") do.
-// A class is cut into slices: runs of at most 32 consecutive positions with at most `cap` T entries and at most
-// `cap` X entries in total (cap >= 31, so a single site always fits).  A slice is one warp's work:
+// Inside a class, every window of 4096 consecutive sites (in breadth-first order) is stably sorted by shape
+// (sg_vb_shape below), so that the sites of a slice almost always share one.
+// A class is cut into slices: runs of at most 32 consecutive positions with at most capE = 32*it entries, of which at
+// most capX = 32*itx X entries (it, itx: per class, chosen by the host from the class's degrees; a single site always
+// fits).  A slice is one warp's work:
 //   hdr[g]           = first position, first index in `col`, first index in the coupling array, and
-//                      n | nTs << 6 | nXs << 16  (sites, T entries, X entries of the slice);
-//   col              = for every slice its T entries in site order (parent first, then children by position), then
-//                      its X entries in site order (by position); the coupling array follows the X order;
+//                      n | nXs << 6 | nE << 16 | shape << 28  (sites, X entries, all entries of the slice, the largest
+//                      shape of its sites);
+//   col              = for every slice ONE run of nE neighbour positions: first its X entries in site order (inside a
+//                      site by position), then its T entries in site order (parent first, then children by position);
+//                      the coupling array follows the X order, so entry e < nXs of the run has coupling j_off + e;
 //   orig_s[32 g + j] = original label of the j-th site of slice g (SG_NONE for j >= n): the Philox counter;
-//   rp_s[32 g + j]   = tOff | xOff << 10 | nT << 20 | nX << 25: where the site's T / X entries start inside the
-//                      slice's T / X run, and how many there are.
-// The kernels read a slice's entries with one lane per ENTRY (every lane busy whatever the degrees, streams
-// coalesced, neighbouring entries gather from neighbouring words), park spin ^ coupling in shared memory, and
+//   rp_s[32 g + j]   = xOff | tOff << 8 | nX << 16 | nT << 21: where the site's X / T entries start inside the slice's
+//                      run (tOff counts from the start of the run, so tOff >= nXs), and how many there are.
+// The kernels read a slice's run with one lane per ENTRY, 32 entries per step (every lane busy whatever the degrees,
+// streams coalesced, neighbouring entries gather from neighbouring words), park spin ^ coupling in shared memory, and
 // finish with one lane per SITE.
 constexpr uint32_t SG_NONE = 0xFFFFFFFFu;
 
@@ -48,14 +53,18 @@ struct VBClass {
     uint64_t n;        // sites in the class
     uint64_t slice0;   // first slice
     uint64_t nslices;
+    uint32_t it;       // entry budget of a slice of this class, in steps of 32 entries (capE = 32 * it)
+    uint32_t itx;      // budget of X entries, in steps of 32 (capX = 32 * itx)
 };
 
 struct alignas(16) SGHdr { uint32_t pos0, col_off, j_off, counts; };
+// shape of a site with nX X entries and nT T entries: which count the kernels run for it
+constexpr uint32_t sg_vb_shape(uint32_t nX, uint32_t nT) { return (nX <= 2 && nT <= 2) ? 0u : (nX <= 4 && nT <= 4) ? 1u : 2u; }
 
 struct VBHostGraph {
     uint64_t N = 0, M = 0;
     uint32_t K = 0, dmax = 0;
-    uint32_t cap = 0;                      // entry budget of a slice (T and X each)
+    uint32_t it_max = 0, itx_max = 0;      // largest per-class budgets (steps of 32 entries)
     bool gauge = true;
     std::vector<uint32_t> eu, ev;          // M edges in generation order (original labels)
     std::vector<uint64_t> row_ptr;         // N+1 (original labels)
@@ -75,7 +84,10 @@ struct VBHostGraph {
 
 // Builds everything above.  Returns false and sets the error string on bad arguments.
 bool sg_build_vb_graph(int model /* SG_MODEL_VB or SG_MODEL_RRBG */, uint64_t N, double c, uint64_t seed, uint32_t n_words, VBHostGraph &g);
-uint32_t sg_vb_slice_cap(uint32_t n_words);   // entry budget of a slice for this number of words per site
+// the (it, itx) budgets the kernels are compiled for, by words per thread G = 4, 2, 1 (W % 4 == 0, W % 2 == 0, else)
+struct VBBudget { uint32_t it, itx; };
+constexpr VBBudget SG_VB_BUDGETS_G1[] = {{4, 3}, {5, 4}, {6, 4}, {8, 6}};
+constexpr VBBudget SG_VB_BUDGET_G2 = {4, 3}, SG_VB_BUDGET_G4 = {4, 2};
 
 std::vector<uint64_t> sg_vb_thresholds(double T, uint32_t dmax);   // thr[0..dmax], thr[0]=0
 std::vector<uint64_t> sg_sk_thresholds(double T, uint64_t N);      // thr[0..N-1]
@@ -90,7 +102,7 @@ struct VBDevice {
     uint32_t *orig_s = nullptr;     // 32 per slice
     uint32_t *rp_s = nullptr;       // 32 per slice
     SGHdr *hdr = nullptr;           // nslices+1
-    uint32_t nslices = 0, cap = 0;
+    uint32_t nslices = 0, it_max = 0, itx_max = 0;
     uint64_t thr_host[32] = {0};    // thresholds thr[k], k=0..31 (beyond dmax = 0): passed to the kernels by value
 };
 

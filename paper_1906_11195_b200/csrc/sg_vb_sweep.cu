@@ -3,20 +3,20 @@
 // (a7) and the drawing of the coupling words (a1).  Conventions: DESIGN.md section 3 (O3, O7, Q14).
 //
 // One warp per (slice, group of G words); layout in sg_internal.h.  Two phases:
-//   1. one lane per row ENTRY of the slice: neighbour index and coupling word from the coalesced streams, gather of
-//      the neighbour's spin word(s), x_e = spin ^ coupling (tree entries: no coupling after the gauge transformation)
-//      parked in shared memory.  Every lane is busy whatever the degrees are; consecutive entries belong to
-//      consecutive sites in breadth-first order, so the lanes of a gather share 128-byte lines and 32-byte sectors.
-//   2. one lane per SITE: m_e = own ^ x_e (bit = bond unsatisfied), u = per-lane sum of the m_e in 5 bit planes
+//   1. one lane per row ENTRY of the slice, 32 entries per step: neighbour index and (X entries) coupling word from the
+//      coalesced streams, gather of the neighbour's spin word(s), x_e = spin ^ coupling (tree entries: no coupling
+//      after the gauge transformation) parked in shared memory.  Every lane is busy whatever the degrees; consecutive
+//      tree entries belong to consecutive sites in breadth-first order, so the lanes of a gather share 128-byte lines.
+//   2. one lane per SITE: m_e = own ^ x_e (bit = bond unsatisfied), u = per-lane sum of the m_e in bit planes
 //      (carry-save adders), one Philox draw r per word shared by its 64 lanes, kstar = #{k >= 1 : r < thr[k]}, flip the
 //      lanes with u >= ceil((d - kstar)/2).  No floating point.
 // G = 4: a thread owns four words of its entry / site: one 32-byte sector per access (LDG.256) and one Philox call for
 // the four words (Q6).
 //
 // Memory behaviour (B200, profiles/): couplings, neighbour indices, labels and row pointers are read once per sweep,
-// coalesced, and stream through L2 (evict_first, no L1 allocation).  The gathers are what bounds the sweep: each costs
-// one L1TEX wavefront per distinct 128-byte line of the warp's request, one L2 sector per distinct 32 bytes and, when
-// it misses L2, a whole line from HBM.
+// coalesced, and stream through L2 (evict_first, no L1 allocation).  The gathers cost one L1TEX wavefront per distinct
+// 128-byte line of the warp's request, one L2 sector per distinct 32 bytes and, when they miss L2, a whole line from
+// HBM.
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -32,16 +32,23 @@ namespace {
 #ifndef SG_BT
 #define SG_BT 128      // threads per CTA = 4 warps = 4 (slice, word group) jobs
 #endif
-#ifndef SG_MINB1
-#define SG_MINB1 10    // resident CTAs per SM the one-word kernel is compiled for
+// resident CTAs per SM the one-word kernels are compiled for, by entry budget (it = 4, 5, 6, 8)
+#ifndef SG_MINB4
+#define SG_MINB4 12
+#endif
+#ifndef SG_MINB5
+#define SG_MINB5 12
+#endif
+#ifndef SG_MINB6
+#define SG_MINB6 12
+#endif
+#ifndef SG_MINB8
+#define SG_MINB8 10
 #endif
 constexpr int WARPS = SG_BT / 32;
 // the never-taken exit in front of griddepcontrol.wait compares against this value: an AND of neighbour positions
 // (all < 2^31 - 2) and SG_NONE fillers can never equal it
 constexpr uint32_t PIN_IMPOSSIBLE = 0x7FFFFFFEu;
-
-// compile-time entry budget of a slice (>= sg_vb_slice_cap of the words it serves) and iterations of 32 entries
-template <int G> struct Cap { static constexpr int value = G == 4 ? 64 : 128; static constexpr int iters = value / 32; };
 
 // index type: 32-bit when every index of the instance fits, else 64-bit
 template <bool WIDE> struct Idx { using type = uint32_t; };
@@ -112,119 +119,152 @@ template <int G> __device__ __forceinline__ Vec<G> sm_load(const uint64_t *s, ui
 }
 
 // ---- phase 1 ------------------------------------------------------------------------------------
-// The stream part: neighbour positions of the slice's T and X entries 32k + lane (SG_NONE beyond the run) and the
-// coupling words of the X entries.  Reads arrays that no kernel writes.
-template <int G, bool WIDE>
+// The stream part: neighbour positions of the slice's entries 32k + lane (SG_NONE beyond the run) and the coupling
+// words of its X entries (the first nXs of the run).  Reads arrays that no kernel writes.
+// IT / ITX: steps of 32 entries / of 32 X entries the slices of the class may need (VBClass::it, itx).
+template <int G, int IT, int ITX, bool WIDE>
 struct Streams {
-    static constexpr int IT = Cap<G>::iters;
-    uint32_t nbT[IT], nbX[IT];
-    Vec<G> jw[IT];
+    uint32_t nb[IT];
+    Vec<G> jw[ITX];
 
     __device__ __forceinline__ void load(const uint32_t *__restrict__ col, const uint64_t *__restrict__ J, SGHdr h, uint32_t W, uint32_t w0, uint64_t pol)
     {
         using I = typename Idx<WIDE>::type;
         const uint32_t lane = threadIdx.x & 31u;
-        const uint32_t nTs = (h.counts >> 6) & 1023u, nXs = h.counts >> 16;
-        const uint32_t *ct = col + h.col_off + lane, *cx = ct + nTs;
+        const uint32_t nXs = (h.counts >> 6) & 1023u, nE = (h.counts >> 16) & 4095u;
+        const uint32_t *c = col + h.col_off + lane;
+        const uint64_t *jp = J + (I)(h.j_off + lane) * W + w0;
 #pragma unroll
         for (int k = 0; k < IT; ++k) {
-            nbT[k] = SG_NONE;
-            if (32u * k < nTs)                                 // warp-uniform: most slices need two iterations
-                if (32u * k + lane < nTs) nbT[k] = ld_stream_u32(ct + 32 * k, pol);
+            nb[k] = SG_NONE;
+            if (32u * k + lane < nE) nb[k] = ld_stream_u32(c + 32 * k, pol);
         }
 #pragma unroll
-        for (int k = 0; k < IT; ++k) {
-            nbX[k] = SG_NONE;
+        for (int k = 0; k < ITX; ++k) {
 #pragma unroll
             for (int g = 0; g < G; ++g) jw[k].v[g] = 0;
-            if (32u * k < nXs && 32u * k + lane < nXs) {
-                nbX[k] = ld_stream_u32(cx + 32 * k, pol);
-                jw[k] = ld_stream_vec<G>(J + (I)(h.j_off + 32u * k + lane) * W + w0, pol);
-            }
+            if (32u * k + lane < nXs) jw[k] = ld_stream_vec<G>(jp + (I)(32u * k) * W, pol);
         }
     }
-    // A value that can never equal PIN_IMPOSSIBLE and is known only when the last stream loads have returned: the
-    // last index and coupling loads of both runs (loads return in order per thread) and the two per-site loads.
+    // A value that can never equal PIN_IMPOSSIBLE and is known only when every stream load has returned.
     __device__ __forceinline__ uint32_t pin(uint32_t site, uint32_t rp) const
     {
-        uint32_t a = nbT[IT - 1] & nbX[IT - 1] & nbT[0] & nbX[0];     // a position (< 2^31 - 2) or SG_NONE
-        a &= (uint32_t)(jw[IT - 1].v[G - 1] >> 32) | (uint32_t)(jw[0].v[0] >> 32) | site | rp | 0x7FFFFFFFu;
-        return a;
+        uint32_t a = nb[0];                                            // AND of positions (< 2^31 - 2) and SG_NONE fillers
+#pragma unroll
+        for (int k = 1; k < IT; ++k) a &= nb[k];
+        uint32_t o = site | rp;
+#pragma unroll
+        for (int k = 0; k < ITX; ++k) o |= (uint32_t)(jw[k].v[G - 1] >> 32) | (uint32_t)jw[k].v[0];
+        return a & (o | 0x7FFFFFFFu);
     }
     // the gather part: x_e = spin[neighbour] (^ coupling) into shared memory; all gathers in flight before the first store
-    __device__ __forceinline__ void gather(const uint64_t *spin, uint32_t W, uint32_t w0, uint64_t *sT, uint64_t *sX) const
+    __device__ __forceinline__ void gather(const uint64_t *spin, uint32_t W, uint32_t w0, uint64_t *sx) const
     {
         using I = typename Idx<WIDE>::type;
         const uint32_t lane = threadIdx.x & 31u;
-        Vec<G> xT[IT], xX[IT];
+        Vec<G> x[IT];
 #pragma unroll
         for (int k = 0; k < IT; ++k)
-            if (nbT[k] != SG_NONE) xT[k] = ld_plain_vec<G>(spin + (I)nbT[k] * W + w0);
+            if (nb[k] != SG_NONE) x[k] = ld_plain_vec<G>(spin + (I)nb[k] * W + w0);
 #pragma unroll
         for (int k = 0; k < IT; ++k)
-            if (nbX[k] != SG_NONE) xX[k] = ld_plain_vec<G>(spin + (I)nbX[k] * W + w0);
+            if (nb[k] != SG_NONE) {
+                if (k < ITX) {
 #pragma unroll
-        for (int k = 0; k < IT; ++k)
-            if (nbT[k] != SG_NONE) sm_store<G>(sT, 32u * k + lane, xT[k]);
-#pragma unroll
-        for (int k = 0; k < IT; ++k)
-            if (nbX[k] != SG_NONE) {
-#pragma unroll
-                for (int g = 0; g < G; ++g) xX[k].v[g] ^= jw[k].v[g];
-                sm_store<G>(sX, 32u * k + lane, xX[k]);
+                    for (int g = 0; g < G; ++g) x[k].v[g] ^= jw[k].v[g];
+                }
+                sm_store<G>(sx, 32u * k + lane, x[k]);
             }
     }
 };
 
 // ---- phase 2 ------------------------------------------------------------------------------------
-// u of the site whose row pointer is rp: its T entries sT[tOff ..], its X entries sX[xOff ..]
+// u of the site whose row pointer is rp: its X entries sx[xOff ..], its T entries sx[tOff ..]
 template <int G>
-__device__ __forceinline__ void count_unsatisfied(const uint64_t *sT, const uint64_t *sX, uint32_t rp, const Vec<G> &own, Planes<G> &P)
+__device__ __forceinline__ void count_unsatisfied(const uint64_t *sx, uint32_t rp, const Vec<G> &own, Planes<G> &P)
 {
-    const uint32_t tOff = rp & 1023u, xOff = (rp >> 10) & 1023u, nT = (rp >> 20) & 31u, nX = rp >> 25;
+    const uint32_t xOff = rp & 255u, tOff = (rp >> 8) & 255u, nX = (rp >> 16) & 31u, nT = rp >> 21;
     Vec<G> mT[4], mX[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
 #pragma unroll
         for (int g = 0; g < G; ++g) mT[q].v[g] = mX[q].v[g] = 0;
-        if ((uint32_t)q < nT) {
-            mT[q] = sm_load<G>(sT, tOff + q);
-#pragma unroll
-            for (int g = 0; g < G; ++g) mT[q].v[g] ^= own.v[g];
-        }
         if ((uint32_t)q < nX) {
-            mX[q] = sm_load<G>(sX, xOff + q);
+            mX[q] = sm_load<G>(sx, xOff + q);
 #pragma unroll
             for (int g = 0; g < G; ++g) mX[q].v[g] ^= own.v[g];
         }
+        if ((uint32_t)q < nT) {
+            mT[q] = sm_load<G>(sx, tOff + q);
+#pragma unroll
+            for (int g = 0; g < G; ++g) mT[q].v[g] ^= own.v[g];
+        }
     }
     planes_from8<G>(P, mT, mX);
-    for (uint32_t q = 4; q < nT; ++q) {           // long rows: per-lane loops, shared memory only
-        Vec<G> m = sm_load<G>(sT, tOff + q);
-#pragma unroll
-        for (int g = 0; g < G; ++g) m.v[g] ^= own.v[g];
-        planes_add1<G>(P, m);
-    }
-    for (uint32_t q = 4; q < nX; ++q) {
-        Vec<G> m = sm_load<G>(sX, xOff + q);
+    // long rows: one per-lane loop over the X entries beyond the fourth, then the T entries beyond the fourth
+    const uint32_t eX = nX > 4u ? nX - 4u : 0u, eT = nT > 4u ? nT - 4u : 0u;
+    for (uint32_t q = 0; q < eX + eT; ++q) {
+        Vec<G> m = sm_load<G>(sx, q < eX ? xOff + 4u + q : tOff + 4u + (q - eX));
 #pragma unroll
         for (int g = 0; g < G; ++g) m.v[g] ^= own.v[g];
         planes_add1<G>(P, m);
     }
 }
 
-// lanes with u >= umin, umin <= 16: the carry out of u + (32 - umin) over the 5 planes, one majority per plane:
-// carry' = maj(plane, carry, k_b) with k_b = bit b of 32 - umin spread over the word (umin = 0: every lane)
-template <int G>
+// The same for a slice whose sites all have at most NS X entries and NS T entries (NS = 2 or 4; shapes 0 and 1 of
+// sg_vb_shape): no loops, u <= 2 NS fits 3 / 4 planes (the planes above stay zero).
+template <int G, int NS>
+__device__ __forceinline__ void count_unsatisfied_short(const uint64_t *sx, uint32_t rp, const Vec<G> &own, Planes<G> &P)
+{
+    const uint32_t xOff = rp & 255u, tOff = (rp >> 8) & 255u, nX = (rp >> 16) & 31u, nT = rp >> 21;
+    Vec<G> mT[4], mX[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+#pragma unroll
+        for (int g = 0; g < G; ++g) mT[q].v[g] = mX[q].v[g] = 0;
+        if (q < NS && (uint32_t)q < nX) {
+            mX[q] = sm_load<G>(sx, xOff + q);
+#pragma unroll
+            for (int g = 0; g < G; ++g) mX[q].v[g] ^= own.v[g];
+        }
+        if (q < NS && (uint32_t)q < nT) {
+            mT[q] = sm_load<G>(sx, tOff + q);
+#pragma unroll
+            for (int g = 0; g < G; ++g) mT[q].v[g] ^= own.v[g];
+        }
+    }
+    if constexpr (NS == 4) {
+        planes_from8<G>(P, mT, mX);
+    } else {
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            const uint64_t a = mX[0].v[g], b = mX[1].v[g], c = mT[0].v[g], d = mT[1].v[g];
+            const uint64_t s = a ^ b ^ c, c1 = maj64(a, b, c), c2 = s & d;
+            P.p[0][g] = s ^ d;
+            P.p[1][g] = c1 ^ c2;
+            P.p[2][g] = c1 & c2;
+            P.p[3][g] = 0;
+            P.p[4][g] = 0;
+        }
+    }
+}
+
+// lanes with u >= umin, for u < 2^NP and umin <= 2^(NP-1): the carry out of u + (2^NP - umin) over the NP planes, one
+// majority per plane: carry' = maj(plane, carry, k_b) with k_b = bit b of 2^NP - umin spread over the word
+// (umin = 0: every lane)
+template <int G, int NP>
 __device__ __forceinline__ uint64_t lanes_ge(const Planes<G> &P, int g, uint32_t umin)
 {
-    const uint32_t K = 32u - umin;
-    uint64_t carry = 0;
+    const uint32_t K = (1u << NP) - umin;
+    uint32_t clo = 0, chi = 0;
 #pragma unroll
-    for (int b = 0; b < 5; ++b) {
-        const uint64_t kb = 0ull - (uint64_t)((K >> b) & 1u);
-        carry = maj64(P.p[b][g], carry, kb);
+    for (int b = 0; b < NP; ++b) {
+        const uint32_t kb = (uint32_t)((int32_t)(K << (31 - b)) >> 31);
+        const uint32_t plo = (uint32_t)P.p[b][g], phi = (uint32_t)(P.p[b][g] >> 32);
+        clo = (plo & clo) | (kb & (plo ^ clo));
+        chi = (phi & chi) | (kb & (phi ^ chi));
     }
+    const uint64_t carry = (uint64_t)chi << 32 | clo;
     return umin == 0 ? ~0ull : carry;
 }
 
@@ -242,14 +282,13 @@ struct SweepArgs {
 };
 
 // W1: one word per site, known at compile time (no index multiplications)
-template <int G, bool WIDE, bool W1, int MINB>
+template <int G, int IT, int ITX, bool WIDE, bool W1, int MINB>
 __global__ void __launch_bounds__(SG_BT, MINB) k_vb_sweep(const __grid_constant__ SweepArgs a)
 {
     using I = typename Idx<WIDE>::type;
     const uint32_t W = W1 ? 1u : a.W, NG = W1 ? 1u : a.NG;
-    constexpr int CAPK = Cap<G>::value;
-    __shared__ __align__(16) uint64_t s_x[WARPS][2 * CAPK * G];
-    uint64_t *sT = s_x[threadIdx.x >> 5], *sX = sT + CAPK * G;
+    __shared__ __align__(16) uint64_t s_x[WARPS][32 * IT * G];
+    uint64_t *sx = s_x[threadIdx.x >> 5];
     // `reverse`: walk the class from its last slice to its first (the host alternates the direction from launch to
     // launch, so that a launch starts where the previous one ended and finds those spin words still in L2)
     const uint32_t bid = a.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
@@ -264,7 +303,7 @@ __global__ void __launch_bounds__(SG_BT, MINB) k_vb_sweep(const __grid_constant_
     const SGHdr h{t.x, t.y, t.z, t.w};
     const uint32_t site = ld_stream_u32(a.orig_s + (gs * 32u + lane), pol);   // SG_NONE: no site in this lane
     const uint32_t rp = ld_stream_u32(a.rp_s + (gs * 32u + lane), pol);
-    Streams<G, WIDE> st;
+    Streams<G, IT, ITX, WIDE> st;
     st.load(a.col, a.J, h, W, w0, pol);
 
     // r = x_{w&3} of P(site, w>>2, sweep, tag 0): the ten Philox rounds run while the stream loads are in flight
@@ -295,20 +334,37 @@ __global__ void __launch_bounds__(SG_BT, MINB) k_vb_sweep(const __grid_constant_
 #pragma unroll
     for (int g = 0; g < G; ++g) own.v[g] = 0;
     if (site != SG_NONE) own = ld_plain_vec<G>(own_ptr);
-    st.gather(a.spin, W, w0, sT, sX);
+    st.gather(a.spin, W, w0, sx);
     __syncwarp();
 
+    // flip <=> kk = d - 2u <= kstar <=> u >= ceil((d - kstar)/2); the slice's shape (warp-uniform) picks the count
     Planes<G> P;
-    count_unsatisfied<G>(sT, sX, rp, own, P);
-    // flip <=> kk = d - 2u <= kstar <=> u >= ceil((d - kstar)/2)
-    const uint32_t d = ((rp >> 20) & 31u) + (rp >> 25);
+    const uint32_t d = ((rp >> 16) & 31u) + (rp >> 21), shape = h.counts >> 28;
     uint64_t any = 0;
+    if (shape == 0) {
+        count_unsatisfied_short<G, 2>(sx, rp, own, P);
 #pragma unroll
-    for (int g = 0; g < G; ++g) {
-        const uint32_t kstar = min(kall[g], d);
-        const uint64_t flip = lanes_ge<G>(P, g, (d - kstar + 1u) >> 1);
-        own.v[g] ^= flip;
-        any |= flip;
+        for (int g = 0; g < G; ++g) {
+            const uint64_t flip = lanes_ge<G, 3>(P, g, (d - min(kall[g], d) + 1u) >> 1);
+            own.v[g] ^= flip;
+            any |= flip;
+        }
+    } else if (shape == 1) {
+        count_unsatisfied_short<G, 4>(sx, rp, own, P);
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            const uint64_t flip = lanes_ge<G, 4>(P, g, (d - min(kall[g], d) + 1u) >> 1);
+            own.v[g] ^= flip;
+            any |= flip;
+        }
+    } else {
+        count_unsatisfied<G>(sx, rp, own, P);
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            const uint64_t flip = lanes_ge<G, 5>(P, g, (d - min(kall[g], d) + 1u) >> 1);
+            own.v[g] ^= flip;
+            any |= flip;
+        }
     }
     if (site != SG_NONE && any) st_plain_vec<G>(own_ptr, own);
 }
@@ -318,6 +374,7 @@ __global__ void __launch_bounds__(SG_BT, MINB) k_vb_sweep(const __grid_constant_
 // One launch over every slice of the instance; grid.y = word; a warp takes UNSAT_ROWS consecutive slices and keeps its
 // per-lane totals in vertical counters, then shared memory, then one atomicAdd per lane and CTA.
 constexpr uint32_t UNSAT_ROWS = 4;
+constexpr int UNSAT_IT = 8, UNSAT_ITX = 6;      // the largest budgets of SG_VB_BUDGETS_G1: serves every class
 
 template <bool WIDE>
 __global__ void __launch_bounds__(SG_BT, 8)
@@ -326,11 +383,10 @@ k_vb_unsat(const uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, co
            unsigned long long *__restrict__ counts)
 {
     using I = typename Idx<WIDE>::type;
-    constexpr int CAPK = Cap<1>::value;
     constexpr int PT = 5 + 2 + 5;      // u <= 31, UNSAT_ROWS additions, 5 doublings in the warp
-    __shared__ __align__(16) uint64_t s_x[WARPS][2 * CAPK];
+    __shared__ __align__(16) uint64_t s_x[WARPS][32 * UNSAT_IT];
     __shared__ unsigned long long s_counts[64];
-    uint64_t *sT = s_x[threadIdx.x >> 5], *sX = sT + CAPK;
+    uint64_t *sx = s_x[threadIdx.x >> 5];
     if (threadIdx.x < 64) s_counts[threadIdx.x] = 0;
     __syncthreads();
     const uint32_t w = blockIdx.y;
@@ -345,15 +401,15 @@ k_vb_unsat(const uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, co
         const uint4 t = __ldg(reinterpret_cast<const uint4 *>(hdr) + slice);
         const SGHdr h{t.x, t.y, t.z, t.w};
         const uint32_t rp = ld_stream_u32(rp_s + slice * 32u + lane, pol);
-        Streams<1, WIDE> st;
+        Streams<1, UNSAT_IT, UNSAT_ITX, WIDE> st;
         st.load(col, J, h, W, w, pol);
         Vec<1> own;
         own.v[0] = 0;
         if (lane < (h.counts & 63u)) own = ld_plain_vec<1>(spin + (I)(h.pos0 + lane) * W + w);
-        st.gather(spin, W, w, sT, sX);
+        st.gather(spin, W, w, sx);
         __syncwarp();
         Planes<1> P;
-        count_unsatisfied<1>(sT, sX, rp, own, P);
+        count_unsatisfied<1>(sx, rp, own, P);
         __syncwarp();
         const uint64_t pl[5] = {P.p[0][0], P.p[1][0], P.p[2][0], P.p[3][0], P.p[4][0]};
         vc_add_planes<5 + 2, PT, 5>(acc, pl);
@@ -377,10 +433,10 @@ k_init_vb_couplings(uint64_t *__restrict__ J, const uint64_t *__restrict__ eps, 
     const SGHdr h = hdr[slice];
     if (lane >= (h.counts & 63u)) return;
     const uint32_t rp = rp_s[slice * 32u + lane];
-    const uint32_t xOff = (rp >> 10) & 1023u, nX = rp >> 25, nTs = (h.counts >> 6) & 1023u;
+    const uint32_t xOff = rp & 255u, nX = (rp >> 16) & 31u;
     const uint64_t p = (uint64_t)h.pos0 + lane;
     for (uint32_t r = 0; r < nX; ++r) {
-        const uint64_t nb = col[(uint64_t)h.col_off + nTs + xOff + r];
+        const uint64_t nb = col[(uint64_t)h.col_off + xOff + r];
         const uint64_t xi = (uint64_t)h.j_off + xOff + r;
         const uint32_t e = jeid[xi];
         for (uint32_t w = 0; w < W; ++w) {
@@ -391,10 +447,9 @@ k_init_vb_couplings(uint64_t *__restrict__ J, const uint64_t *__restrict__ eps, 
     }
 }
 
-template <int G, bool WIDE, bool W1, int MINB>
+template <int G, int IT, int ITX, bool WIDE, bool W1, int MINB>
 int launch(const VBDevice &d, const VBClass &c, uint32_t W, uint32_t word0, uint64_t sweep, SGSeed key, bool reverse, cudaStream_t st)
 {
-    if (d.cap > (uint32_t)Cap<G>::value) { sg_set_error("k_vb_sweep: the slice budget of the instance exceeds the kernel's"); return SG_EINVAL; }
     SweepArgs a;
     a.spin = d.spin; a.J = d.J; a.col = d.col; a.orig_s = d.orig_s; a.rp_s = d.rp_s; a.hdr = d.hdr;
     for (int k = 0; k < 32; ++k) a.thr[k] = d.thr_host[k];
@@ -415,7 +470,7 @@ int launch(const VBDevice &d, const VBClass &c, uint32_t W, uint32_t word0, uint
     cfg.attrs = attr;
     static const bool no_pdl = std::getenv("SG_NO_PDL") != nullptr;   // measurement knob
     cfg.numAttrs = no_pdl ? 0 : 1;
-    const cudaError_t le = cudaLaunchKernelEx(&cfg, k_vb_sweep<G, WIDE, W1, MINB>, a);
+    const cudaError_t le = cudaLaunchKernelEx(&cfg, k_vb_sweep<G, IT, ITX, WIDE, W1, MINB>, a);
     sgk_count_launch();
     const cudaError_t e = le != cudaSuccess ? le : cudaGetLastError();
     if (e != cudaSuccess) {
@@ -423,6 +478,18 @@ int launch(const VBDevice &d, const VBClass &c, uint32_t W, uint32_t word0, uint
         return SG_ECUDA;
     }
     return SG_OK;
+}
+
+// one word per thread: the class's budget picks the instantiation (SG_VB_BUDGETS_G1)
+template <bool WIDE, bool W1>
+int launch_g1(const VBDevice &d, const VBClass &c, uint32_t W, uint32_t word0, uint64_t sweep, SGSeed key, bool reverse, cudaStream_t st)
+{
+    if (c.it <= 4 && c.itx <= 3) return launch<1, 4, 3, WIDE, W1, SG_MINB4>(d, c, W, word0, sweep, key, reverse, st);
+    if (c.it <= 5 && c.itx <= 4) return launch<1, 5, 4, WIDE, W1, SG_MINB5>(d, c, W, word0, sweep, key, reverse, st);
+    if (c.it <= 6 && c.itx <= 4) return launch<1, 6, 4, WIDE, W1, SG_MINB6>(d, c, W, word0, sweep, key, reverse, st);
+    if (c.it <= 8 && c.itx <= 6) return launch<1, 8, 6, WIDE, W1, SG_MINB8>(d, c, W, word0, sweep, key, reverse, st);
+    sg_set_error("k_vb_sweep: the slice budget of the class exceeds the kernels'");
+    return SG_EINVAL;
 }
 
 // test knob (read at every launch, so that one process can exercise both paths): 64-bit index arithmetic on any instance
@@ -437,18 +504,18 @@ int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint64_t N, uint64_t
     const bool wide = force_wide() || N * W >= (1ull << 32) || nJ * W >= (1ull << 32);
     const uint32_t G = (W % 4 == 0) ? 4 : (W % 2 == 0) ? 2 : 1;
     if (c.nslices * (uint64_t)(W / G) >= (1ull << 31)) { sg_set_error("sgk_vb_sweep_class: class too large"); return SG_EINVAL; }
+    if (G != 1 && (c.it > 4 || c.itx > (G == 2 ? 3u : 2u))) { sg_set_error("k_vb_sweep: the slice budget of the class exceeds the kernels'"); return SG_EINVAL; }
     if (!wide) {
         switch (G) {
-        case 1: return W == 1 ? launch<1, false, true, SG_MINB1>(d, c, W, word0, sweep, key, reverse, st)
-                              : launch<1, false, false, SG_MINB1>(d, c, W, word0, sweep, key, reverse, st);
-        case 2: return launch<2, false, false, 6>(d, c, W, word0, sweep, key, reverse, st);
-        default: return launch<4, false, false, 4>(d, c, W, word0, sweep, key, reverse, st);
+        case 1: return W == 1 ? launch_g1<false, true>(d, c, W, word0, sweep, key, reverse, st) : launch_g1<false, false>(d, c, W, word0, sweep, key, reverse, st);
+        case 2: return launch<2, 4, 3, false, false, 6>(d, c, W, word0, sweep, key, reverse, st);
+        default: return launch<4, 4, 2, false, false, 4>(d, c, W, word0, sweep, key, reverse, st);
         }
     }
     switch (G) {
-    case 1: return launch<1, true, false, SG_MINB1>(d, c, W, word0, sweep, key, reverse, st);
-    case 2: return launch<2, true, false, 6>(d, c, W, word0, sweep, key, reverse, st);
-    default: return launch<4, true, false, 4>(d, c, W, word0, sweep, key, reverse, st);
+    case 1: return launch_g1<true, false>(d, c, W, word0, sweep, key, reverse, st);
+    case 2: return launch<2, 4, 3, true, false, 6>(d, c, W, word0, sweep, key, reverse, st);
+    default: return launch<4, 4, 2, true, false, 4>(d, c, W, word0, sweep, key, reverse, st);
     }
 }
 
@@ -456,7 +523,7 @@ int sgk_vb_unsat(const VBDevice &d, uint64_t N, uint64_t nJ, uint32_t W, uint64_
 {
     const uint64_t nslices = d.nslices;
     if (nslices == 0) return SG_OK;
-    if (d.cap > (uint32_t)Cap<1>::value) { sg_set_error("k_vb_unsat: the slice budget of the instance exceeds the kernel's"); return SG_EINVAL; }
+    if (d.it_max > (uint32_t)UNSAT_IT || d.itx_max > (uint32_t)UNSAT_ITX) { sg_set_error("k_vb_unsat: the slice budget of the instance exceeds the kernel's"); return SG_EINVAL; }
     const bool wide = force_wide() || N * W >= (1ull << 32) || nJ * W >= (1ull << 32);
     const uint64_t warps = (nslices + UNSAT_ROWS - 1) / UNSAT_ROWS;
     dim3 grid((unsigned)((warps + WARPS - 1) / WARPS), W);

@@ -92,12 +92,17 @@ def _decode_rows(g):
     X = [[] for _ in range(N)]
     label = np.full(N, -1, dtype=np.int64)
     hdr = g["hdr"].astype(np.int64)
+    it_of = np.zeros(g["nslices"], dtype=np.int64)
+    itx_of = np.zeros(g["nslices"], dtype=np.int64)
+    for k in range(g["K"]):
+        s0, ns = int(g["class_slice0"][k]), int(g["class_nslices"][k])
+        it_of[s0:s0 + ns] = int(g["class_it"][k]); itx_of[s0:s0 + ns] = int(g["class_itx"][k])
     for s_ in range(g["nslices"]):
         pos0, col_off, j_off, counts = hdr[s_]
-        n, nTs, nXs = counts & 63, (counts >> 6) & 1023, counts >> 16
-        assert 1 <= n <= 32 and nTs <= g["cap"] and nXs <= g["cap"]
-        assert hdr[s_ + 1][1] == col_off + nTs + nXs and hdr[s_ + 1][2] == j_off + nXs
-        t_run, x_run = 0, 0
+        n, nXs, nE = counts & 63, (counts >> 6) & 1023, (counts >> 16) & 4095
+        assert 1 <= n <= 32 and nE <= 32 * it_of[s_] and nXs <= 32 * itx_of[s_] and nXs <= nE
+        assert hdr[s_ + 1][1] == col_off + nE and hdr[s_ + 1][2] == j_off + nXs
+        x_run, t_run = 0, nXs                                      # one run: the X entries, then the T entries
         for j in range(32):
             rp = int(g["rp_s"][32 * s_ + j])
             if j >= n:
@@ -105,12 +110,12 @@ def _decode_rows(g):
                 continue
             p = pos0 + j
             label[p] = int(g["orig_s"][32 * s_ + j])
-            tOff, xOff, nT, nX = rp & 1023, (rp >> 10) & 1023, (rp >> 20) & 31, rp >> 25
+            xOff, tOff, nX, nT = rp & 255, (rp >> 8) & 255, (rp >> 16) & 31, rp >> 21
             assert tOff == t_run and xOff == x_run                 # site order, no gaps
             T[p] = [int(q) for q in g["col"][col_off + tOff:col_off + tOff + nT]]
-            X[p] = [(int(g["col"][col_off + nTs + xOff + r]), int(j_off + xOff + r)) for r in range(nX)]
+            X[p] = [(int(g["col"][col_off + xOff + r]), int(j_off + xOff + r)) for r in range(nX)]
             t_run += nT; x_run += nX
-        assert t_run == nTs and x_run == nXs
+        assert x_run == nXs and t_run == nE
     return T, X, label
 
 
@@ -130,18 +135,28 @@ def test_host_generator_matches_oracle_and_layout_is_consistent(sg, oracle_mod, 
     _, _, colour = o.graph()
     assert np.array_equal(g["colour"], colour)
     NONE = 0xFFFFFFFF
-    K, cap = g["K"], g["cap"]
-    assert g["gauge"] == 1 and cap == (64 if W % 4 == 0 else 128)
+    K = g["K"]
+    assert g["gauge"] == 1
     orig = g["orig"].astype(np.int64)
     assert np.array_equal(np.sort(orig), np.arange(N))
     pos = np.empty(N, dtype=np.int64)
     pos[orig] = np.arange(N)
     degree = np.bincount(e.ravel().astype(np.int64), minlength=N)
     rows, order, par, par_e = _bfs_forest(N, e)
-    # positions: class-major; breadth-first order inside a class
+    # positions: class-major; inside a class breadth-first order, every window of 4096 sites stably sorted by shape
+    # (0: at most 2 X and 2 T entries, 1: at most 4 and 4, 2: longer rows; T = forest edges, X = the others)
+    nT_lab = np.zeros(N, dtype=np.int64)
+    for i in range(N):
+        if par[i] >= 0:
+            nT_lab[i] += 1; nT_lab[par[i]] += 1
+
+    def shape(nx, nt):
+        return 0 if (nx <= 2 and nt <= 2) else 1 if (nx <= 4 and nt <= 4) else 2
     p0 = 0
     for k in range(K):
         members = [i for i in order if colour[i] == k]
+        members = [i for a in range(0, len(members), 4096)
+                   for i in sorted(members[a:a + 4096], key=lambda i: shape(degree[i] - nT_lab[i], nT_lab[i]))]
         assert int(g["class_pos0"][k]) == p0 and int(g["class_n"][k]) == len(members)
         assert orig[p0:p0 + len(members)].tolist() == members
         p0 += len(members)
@@ -174,23 +189,34 @@ def test_host_generator_matches_oracle_and_layout_is_consistent(sg, oracle_mod, 
     is_tree[[k for k in par_e if k >= 0]] = True
     assert np.all(seen_edges[~is_tree] == 2) and np.all(seen_edges[is_tree] == 0)
     assert g["entries"] == 2 * g["M"] and g["nJ"] == 2 * int((~is_tree).sum())
-    # slices: greedy cut of every class into runs of <= 32 sites within the entry budget, never across classes
+    # slices: greedy cut of every class into runs of <= 32 sites within the class's budgets (32*it entries, 32*itx X
+    # entries), never across classes; the budget is the one of include/sg.h's list that minimises slices * (200 + 13 it)
+    def cut(k, it, itx):
+        runs = []
+        p, pend = int(g["class_pos0"][k]), int(g["class_pos0"][k]) + int(g["class_n"][k])
+        while p < pend:
+            n = sE = sX = 0
+            while p + n < pend and n < 32:
+                d_, x = degree[orig[p + n]], degree[orig[p + n]] - nT[p + n]
+                if n > 0 and (sE + d_ > 32 * it or sX + x > 32 * itx):
+                    break
+                sE += d_; sX += x; n += 1
+            runs.append((p, n, sX, sE))
+            p += n
+        return runs
+    budgets = [(4, 3), (5, 4), (6, 4), (8, 6)] if W % 2 else [(4, 3)] if W % 4 else [(4, 2)]
     hdr = g["hdr"].astype(np.int64)
     s_ = 0
     for k in range(K):
         assert int(g["class_slice0"][k]) == s_
-        p, pend = int(g["class_pos0"][k]), int(g["class_pos0"][k]) + int(g["class_n"][k])
-        while p < pend:
-            n = sT = sX = 0
-            while p + n < pend and n < 32:
-                t, x = nT[p + n], degree[orig[p + n]] - nT[p + n]
-                if n > 0 and (sT + t > cap or sX + x > cap):
-                    break
-                sT += t; sX += x; n += 1
-            assert hdr[s_][0] == p and hdr[s_][3] == (n | sT << 6 | sX << 16)
-            p += n; s_ += 1
+        best = min(budgets, key=lambda b_: (len(cut(k, *b_)) * (200 + 13 * b_[0]), budgets.index(b_)))
+        assert (int(g["class_it"][k]), int(g["class_itx"][k])) == best
+        for p, n, sX, sE in cut(k, *best):
+            sh = max(shape(degree[orig[q]] - nT[q], nT[q]) for q in range(p, p + n))
+            assert hdr[s_][0] == p and hdr[s_][3] == (n | sX << 6 | sE << 16 | sh << 28)
+            s_ += 1
         assert int(g["class_nslices"][k]) == s_ - int(g["class_slice0"][k])
-    assert s_ == g["nslices"] and hdr[s_][0] == N
+    assert s_ == g["nslices"] and hdr[s_][0] == N and g["it_max"] == max(int(x) for x in g["class_it"])
     # no edge inside a colour class (the race-freedom condition of the parallel update)
     assert np.all(colour[e[:, 0]] != colour[e[:, 1]])
 
