@@ -51,19 +51,6 @@ __device__ __forceinline__ uint64_t policy_evict_first()
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
     return p;
 }
-__device__ __forceinline__ uint64_t policy_evict_last()
-{
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
-// 16 bytes that every sweep reads again and that should stay in L2 (slice headers: 16 bytes per 32 sites)
-__device__ __forceinline__ uint4 ld_keep_u128(const void *ptr, uint64_t pol)
-{
-    uint4 v;
-    asm volatile("ld.global.nc.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(ptr), "l"(pol));
-    return v;
-}
 __device__ __forceinline__ uint32_t ld_stream_u32(const uint32_t *ptr, uint64_t pol)
 {
     uint32_t v;
@@ -88,7 +75,13 @@ __device__ __forceinline__ uint64_t ld_plain_u64(const uint64_t *ptr)
     asm volatile("ld.global.b64 %0, [%1];" : "=l"(v) : "l"(ptr));
     return v;
 }
-
+// a spin word that is read once in this launch (gather along a non-tree edge): cached in L2 only
+__device__ __forceinline__ uint64_t ld_x_u64(const uint64_t *ptr)
+{
+    uint64_t v;
+    asm volatile("ld.global.cg.b64 %0, [%1];" : "=l"(v) : "l"(ptr));
+    return v;
+}
 // vector forms: 8, 16 or 32 bytes per access (LDG.64 / LDG.128 / LDG.256 on sm_100a); ptr aligned to 8*G bytes
 template <int G> __device__ __forceinline__ Vec<G> ld_stream_vec(const uint64_t *ptr, uint64_t pol);
 template <> __device__ __forceinline__ Vec<1> ld_stream_vec<1>(const uint64_t *ptr, uint64_t pol)

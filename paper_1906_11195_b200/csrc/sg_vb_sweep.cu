@@ -158,14 +158,23 @@ struct Streams {
         return a & (o | 0x7FFFFFFFu);
     }
     // the gather part: x_e = spin[neighbour] (^ coupling) into shared memory; all gathers in flight before the first store
-    __device__ __forceinline__ void gather(const uint64_t *spin, uint32_t W, uint32_t w0, uint64_t *sx) const
+    __device__ __forceinline__ void gather(const uint64_t *spin, uint32_t W, uint32_t w0, uint64_t *sx, uint32_t nXs) const
     {
         using I = typename Idx<WIDE>::type;
         const uint32_t lane = threadIdx.x & 31u;
         Vec<G> x[IT];
 #pragma unroll
         for (int k = 0; k < IT; ++k)
-            if (nb[k] != SG_NONE) x[k] = ld_plain_vec<G>(spin + (I)nb[k] * W + w0);
+            if (nb[k] != SG_NONE) {
+                // X entries: one word of a random line, no reuse: kept out of L1 (.cg), which is measurably better than
+                // any L1 hint (profiles/r02_sweep.md); T entries: neighbouring lanes, steps and slices share lines
+                if constexpr (G == 1) {
+                    if (k < ITX && 32u * k + lane < nXs) x[k].v[0] = ld_x_u64(spin + (I)nb[k] * W + w0);
+                    else x[k].v[0] = ld_plain_u64(spin + (I)nb[k] * W + w0);
+                } else {
+                    x[k] = ld_plain_vec<G>(spin + (I)nb[k] * W + w0);
+                }
+            }
 #pragma unroll
         for (int k = 0; k < IT; ++k)
             if (nb[k] != SG_NONE) {
@@ -334,7 +343,7 @@ __global__ void __launch_bounds__(SG_BT, MINB) k_vb_sweep(const __grid_constant_
 #pragma unroll
     for (int g = 0; g < G; ++g) own.v[g] = 0;
     if (site != SG_NONE) own = ld_plain_vec<G>(own_ptr);
-    st.gather(a.spin, W, w0, sx);
+    st.gather(a.spin, W, w0, sx, (h.counts >> 6) & 1023u);
     __syncwarp();
 
     // flip <=> kk = d - 2u <= kstar <=> u >= ceil((d - kstar)/2); the slice's shape (warp-uniform) picks the count
@@ -406,7 +415,7 @@ k_vb_unsat(const uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, co
         Vec<1> own;
         own.v[0] = 0;
         if (lane < (h.counts & 63u)) own = ld_plain_vec<1>(spin + (I)(h.pos0 + lane) * W + w);
-        st.gather(spin, W, w, sx);
+        st.gather(spin, W, w, sx, (h.counts >> 6) & 1023u);
         __syncwarp();
         Planes<1> P;
         count_unsatisfied<1>(sx, rp, own, P);
@@ -462,6 +471,16 @@ int launch(const VBDevice &d, const VBClass &c, uint32_t W, uint32_t word0, uint
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)((jobs + WARPS - 1) / WARPS));
     cfg.blockDim = dim3(SG_BT);
+    // Shared-memory carve-out: 64 KiB (28 % of 228), enough for 10 resident CTAs of the common instantiations, so that
+    // 192 KiB stay L1.  The gathers keep thousands of lines in flight per SM and L1 is where they land: with the
+    // driver's default choice (about 100 KiB of shared memory) the sweep is 3.5 % slower, with a 228 KiB carve-out
+    // 2.5 x slower; 32 KiB (6 CTAs) is 5 % slower (profiles/r02_sweep.md).  SG_VB_CARVEOUT=<percent>: measurement knob.
+    static const int carve_pct = std::getenv("SG_VB_CARVEOUT") ? std::atoi(std::getenv("SG_VB_CARVEOUT")) : 28;
+    static bool carved = false;             // per instantiation
+    if (!carved) {
+        cudaFuncSetAttribute(k_vb_sweep<G, IT, ITX, WIDE, W1, MINB>, cudaFuncAttributePreferredSharedMemoryCarveout, carve_pct);
+        carved = true;
+    }
     cfg.dynamicSmemBytes = 0;
     cfg.stream = st;
     cudaLaunchAttribute attr[1];

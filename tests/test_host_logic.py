@@ -143,8 +143,13 @@ def test_host_generator_matches_oracle_and_layout_is_consistent(sg, oracle_mod, 
     pos[orig] = np.arange(N)
     degree = np.bincount(e.ravel().astype(np.int64), minlength=N)
     rows, order, par, par_e = _bfs_forest(N, e)
-    # positions: class-major; inside a class breadth-first order, every window of 4096 sites stably sorted by shape
-    # (0: at most 2 X and 2 T entries, 1: at most 4 and 4, 2: longer rows; T = forest edges, X = the others)
+    # positions: class-major; inside a class breadth-first order, every window of 4096 sites stably sorted by
+    # (demand, shape); demand 0: a neighbour in a class of fewer than N/32 sites, 1: fewer than N/8, 2: neither;
+    # shape 0: at most 2 X and 2 T entries, 1: at most 4 and 4, 2: longer rows (T = forest edges, X = the others)
+    csize = np.bincount(colour, minlength=K)
+
+    def demand(i):
+        return min([2] + [0 if 32 * csize[colour[v_]] < N else 1 if 8 * csize[colour[v_]] < N else 2 for v_, _ in rows[i]])
     nT_lab = np.zeros(N, dtype=np.int64)
     for i in range(N):
         if par[i] >= 0:
@@ -156,7 +161,7 @@ def test_host_generator_matches_oracle_and_layout_is_consistent(sg, oracle_mod, 
     for k in range(K):
         members = [i for i in order if colour[i] == k]
         members = [i for a in range(0, len(members), 4096)
-                   for i in sorted(members[a:a + 4096], key=lambda i: shape(degree[i] - nT_lab[i], nT_lab[i]))]
+                   for i in sorted(members[a:a + 4096], key=lambda i: (demand(i), shape(degree[i] - nT_lab[i], nT_lab[i])))]
         assert int(g["class_pos0"][k]) == p0 and int(g["class_n"][k]) == len(members)
         assert orig[p0:p0 + len(members)].tolist() == members
         p0 += len(members)
