@@ -118,6 +118,17 @@ def cpu_sample(args, sweeps):
     return n * 64 * args.n_words * sweeps / dt, dt, n
 
 
+def cpu_sample_other(model, n, c, T, sweeps, clones=1):
+    """The other two samples of BASELINE.md section 3: config 1 in full, the SK instance of config 4 for a few sweeps."""
+    import oracle
+
+    o = oracle.Oracle(model, n, c, T, 1, 1, n_clones=clones) if clones > 1 else oracle.Oracle(model, n, c, T, 1, 1)
+    t0 = time.perf_counter()
+    o.sweep(sweeps)
+    dt = time.perf_counter() - t0
+    return n * 64 * clones * sweeps / dt, dt
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores; each step = 1 sweep of the N=2^22 sample."""
     rank, world, _ = dist_setup(args.gpus)
@@ -309,23 +320,48 @@ def run_ours(args):
     if windowed:
         out["windowed"] = windowed
     tr = os.path.join(ROOT, "profiles", "traffic.json")
-    headline = args.model == "vb" and args.log2n == 24 and W == 1
-    if os.path.exists(tr) and headline:      # ncu dram bytes of one sweep of exactly this workload (profiles/r01_sweep.md)
-        out["roofline"]["traffic"] = json.load(open(tr)).get("dram_bytes_per_sweep")
+    headline = args.model == "vb" and args.log2n == 24 and W == 1 and args.T == 1.0
+    if os.path.exists(tr) and headline:
+        # ncu counters of one sweep of exactly this workload, captured once per kernel change and stored under profiles/
+        # (a run under ncu is never a bench run): quoted here, not measured in this run
+        t = json.load(open(tr))
+        out["roofline"]["traffic"] = t.get("dram_bytes_per_sweep")
+        out["roofline"]["traffic_source"] = "profiles/traffic.json (ncu --set full capture of this workload, quoted)"
         out["roofline"]["per"] = "sweep (the K colour-class launches): achieved, traffic and sweep_ms are per sweep"
         out["roofline"]["dram_bytes_per_site_word"] = out["roofline"]["traffic"] / (N * W)       # ncu, BASELINE.md section 2
-        out["roofline"]["frac_104B"] = out["roofline"]["frac"] * 104.0 / 80.0                    # + indices, row pointer, label
-        out["roofline"]["philox_alu_ceiling_spin_updates_per_s"] = 5.79e11 * 64                  # profiles/r01_probes.md
+        if t.get("warp_instructions_per_sweep") and clocks and clocks.get("sm_max_mhz"):
+            # the ALU ceiling of BASELINE.json: the kernel's whole instruction stream (Philox + bit-sliced arithmetic +
+            # addressing) at 4 warp instructions per SM and clock
+            issue = 148 * 4 * clocks["sm_max_mhz"] * 1e6
+            out["roofline"]["alu_ceiling"] = {"value": N * 64 * W / (t["warp_instructions_per_sweep"] / issue), "unit": "spin updates/s",
+                                              "warp_instructions_per_sweep": t["warp_instructions_per_sweep"],
+                                              "source": "profiles/traffic.json smsp__inst_executed.sum (quoted); 148 SMs x 4 issue slots x sm_max_mhz"}
     if not headline:
         out["config"]["l2"] = "not the headline workload: see DESIGN.md section 10"
     if args.model == "sk":
         out["roofline"] = {"bound": "latency", "kernel": "k_sk_sweep", "achieved": None, "peak": None, "unit": None, "frac": None, "traffic": None,
                            "note": "sequential sweep of one instance per CTA (PAPER.md:233): dependency-latency bound, absolute rate only",
                            "sweep_ms": sweep_ms / (SWEEPS_PER_STEP * args.steps)}
-    if not args.no_cpu_baseline and args.model == "vb":   # the headline ensemble only
+    if not args.no_cpu_baseline and args.model == "vb":   # the headline ensemble
         v, dt, n = cpu_sample(args, 2)
         out["cpu_baseline"] = {"value": v, "unit": "spin updates/s", "cores": 1, "kind": "oracle", "host_cores": os.cpu_count(),
-                               "sample": f"same recipe at N=2^{n.bit_length() - 1}, 2 oracle sweeps, {dt:.1f} s"}
+                               "sample": f"same recipe at N=2^{n.bit_length() - 1}, 2 oracle sweeps, {dt:.1f} s (N=2^24 itself would take "
+                                         "about 35 s per sweep plus 40 s of setup on one core: the rate per site does not depend on N)"}
+        if headline:                                      # the other two samples of BASELINE.md section 3
+            import oracle
+
+            v1, d1 = cpu_sample_other(oracle.VB, 1024, 4.0, 1.0, 1024)
+            v4, d4 = cpu_sample_other(oracle.SK, 4096, 0.0, 0.6, 2)
+            out["cpu_baseline"]["also"] = [
+                {"value": v1, "unit": "spin updates/s", "sample": f"BASELINE.json configs[0] in full: VB N=1024, 1024 sweeps, {d1:.1f} s"},
+                {"value": v4, "unit": "spin updates/s", "sample": f"BASELINE.json configs[3]: SK N=4096 T=0.6, 2 sweeps, {d4:.1f} s"}]
+    if not args.no_cpu_baseline and args.model == "sk":
+        import oracle
+
+        n = 1 << min(12, args.log2n)
+        v4, d4 = cpu_sample_other(oracle.SK, n, 0.0, args.T, 2, args.clones)
+        out["cpu_baseline"] = {"value": v4, "unit": "spin updates/s", "cores": 1, "kind": "oracle", "host_cores": os.cpu_count(),
+                               "sample": f"SK N={n} T={args.T}, {args.clones} clone(s), 2 oracle sweeps, {d4:.1f} s"}
     out["context"] = {"paper": "~15 ps per spin update on one P100 = 6.7e10 spin updates/s (PAPER.md:320); "
                                "total work of the order of 2^64 spin updates (PAPER.md:165)"}
     print(json.dumps(out))

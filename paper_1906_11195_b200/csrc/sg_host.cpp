@@ -313,8 +313,8 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t 
         const uint32_t i = g.orig[p];
         if (par[i] != SG_NONE) { g.tpar[p] = g.pos[par[i]]; g.teid[p] = par_e[i]; }
     }
-    // per-class entry budgets (sg_internal.h): among the budgets the kernels are compiled for, the one that minimises
-    // an estimate of the warp instructions per site, slices * (fixed part + per-step part * it)
+    // per-class entry budgets (sg_internal.h): the smallest budget the kernels are compiled for whose greedy cut needs at
+    // most 5 % more slices than the largest budget's (measured: fewer, fuller slices beat shorter unrolled loops)
     // (SG_VB_IT=<it> forces one budget for all classes: a measurement knob; outputs are identical)
     const char *it_env = std::getenv("SG_VB_IT");
     auto count_slices = [&](uint32_t k, VBBudget bud) {
@@ -336,14 +336,14 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t 
     for (uint32_t k = 0; k < K; ++k) {
         VBBudget best = n_words % 4 == 0 ? SG_VB_BUDGET_G4 : SG_VB_BUDGET_G2;
         if (n_words % 2 != 0) {
-            double best_cost = 0;
-            bool first = true;
-            for (const VBBudget bud : SG_VB_BUDGETS_G1) {
-                if (it_env && (uint32_t)std::atoi(it_env) != bud.it) continue;
-                const double cost = (double)count_slices(k, bud) * (200.0 + 13.0 * bud.it);
-                if (first || cost < best_cost) { best = bud; best_cost = cost; first = false; }
-            }
-            if (first) best = SG_VB_BUDGETS_G1[0];
+            constexpr size_t NB = sizeof(SG_VB_BUDGETS_G1) / sizeof(SG_VB_BUDGETS_G1[0]);
+            best = SG_VB_BUDGETS_G1[NB - 1];
+            const uint64_t fewest = count_slices(k, best);
+            for (size_t b = 0; b + 1 < NB; ++b)
+                if (count_slices(k, SG_VB_BUDGETS_G1[b]) * 100 <= fewest * 105) { best = SG_VB_BUDGETS_G1[b]; break; }
+            if (it_env)
+                for (const VBBudget bud : SG_VB_BUDGETS_G1)
+                    if ((uint32_t)std::atoi(it_env) == bud.it) best = bud;
         }
         g.cls[k].it = best.it; g.cls[k].itx = best.itx;
         g.it_max = std::max(g.it_max, best.it); g.itx_max = std::max(g.itx_max, best.itx);

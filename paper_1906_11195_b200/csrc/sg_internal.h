@@ -29,11 +29,13 @@ Philox4 sg_philox_host(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint3
 // s_i -> eps_i s_i, J_ij -> eps_i J_ij eps_j with eps_child = eps_parent * J_(parent,child) (eps_root = +1), which
 // changes no bond state, hence no flip decision, energy or correlation count.  The device stores the
 // transformed spins and couplings; tree entries ("T") need no coupling word at all, the others ("X") do.
-// Inside a class, every window of 4096 consecutive sites (in breadth-first order) is stably sorted by shape
-// (sg_vb_shape below), so that the sites of a slice almost always share one.
+// Inside a class, every window of 4096 consecutive sites (in breadth-first order) is stably sorted by (demand, shape):
+// demand 0 = the site has a neighbour in a class of fewer than N/32 sites, 1 = in a class of fewer than N/8 sites,
+// 2 = neither (the gathers of the small classes then use whole lines); shape = sg_vb_shape below, so that the sites of a
+// slice almost always share one.
 // A class is cut into slices: runs of at most 32 consecutive positions with at most capE = 32*it entries, of which at
-// most capX = 32*itx X entries (it, itx: per class, chosen by the host from the class's degrees; a single site always
-// fits).  A slice is one warp's work:
+// most capX = 32*itx X entries (it, itx: per class, the smallest budget the kernels are compiled for that needs at most
+// 5 % more slices than the largest one; a single site always fits).  A slice is one warp's work:
 //   hdr[g]           = first position, first index in `col`, first index in the coupling array, and
 //                      n | nXs << 6 | nE << 16 | shape << 28  (sites, X entries, all entries of the slice, the largest
 //                      shape of its sites);
@@ -86,7 +88,7 @@ struct VBHostGraph {
 bool sg_build_vb_graph(int model /* SG_MODEL_VB or SG_MODEL_RRBG */, uint64_t N, double c, uint64_t seed, uint32_t n_words, VBHostGraph &g);
 // the (it, itx) budgets the kernels are compiled for, by words per thread G = 4, 2, 1 (W % 4 == 0, W % 2 == 0, else)
 struct VBBudget { uint32_t it, itx; };
-constexpr VBBudget SG_VB_BUDGETS_G1[] = {{4, 3}, {5, 4}, {6, 4}, {8, 6}};
+constexpr VBBudget SG_VB_BUDGETS_G1[] = {{6, 4}, {8, 6}};
 constexpr VBBudget SG_VB_BUDGET_G2 = {4, 3}, SG_VB_BUDGET_G4 = {4, 2};
 
 std::vector<uint64_t> sg_vb_thresholds(double T, uint32_t dmax);   // thr[0..dmax], thr[0]=0
@@ -136,9 +138,5 @@ struct SKDevice {
     uint32_t nthr_nz = 0;
     bool accept_all = false;     // T = inf
 };
-int sgk_sk_init_rows(const SKDevice &d, uint64_t N, uint32_t W, SGSeed key, cudaStream_t st);
-int sgk_sk_init_fields(const SKDevice &d, uint64_t N, uint32_t W, cudaStream_t st);
-int sgk_sk_sweep(const SKDevice &d, uint64_t N, uint32_t W, uint64_t sweep, uint64_t nsweeps, SGSeed key, cudaStream_t st);
-int sgk_sk_energy(const SKDevice &d, uint64_t N, uint32_t W, int64_t *out_dev, cudaStream_t st);
 
 uint64_t sgk_launch_count();

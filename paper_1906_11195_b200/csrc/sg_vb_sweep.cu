@@ -32,13 +32,7 @@ namespace {
 #ifndef SG_BT
 #define SG_BT 128      // threads per CTA = 4 warps = 4 (slice, word group) jobs
 #endif
-// resident CTAs per SM the one-word kernels are compiled for, by entry budget (it = 4, 5, 6, 8)
-#ifndef SG_MINB4
-#define SG_MINB4 12
-#endif
-#ifndef SG_MINB5
-#define SG_MINB5 12
-#endif
+// resident CTAs per SM the one-word kernels are compiled for, by entry budget (it = 6, 8): 40 / 48 registers
 #ifndef SG_MINB6
 #define SG_MINB6 12
 #endif
@@ -503,8 +497,6 @@ int launch(const VBDevice &d, const VBClass &c, uint32_t W, uint32_t word0, uint
 template <bool WIDE, bool W1>
 int launch_g1(const VBDevice &d, const VBClass &c, uint32_t W, uint32_t word0, uint64_t sweep, SGSeed key, bool reverse, cudaStream_t st)
 {
-    if (c.it <= 4 && c.itx <= 3) return launch<1, 4, 3, WIDE, W1, SG_MINB4>(d, c, W, word0, sweep, key, reverse, st);
-    if (c.it <= 5 && c.itx <= 4) return launch<1, 5, 4, WIDE, W1, SG_MINB5>(d, c, W, word0, sweep, key, reverse, st);
     if (c.it <= 6 && c.itx <= 4) return launch<1, 6, 4, WIDE, W1, SG_MINB6>(d, c, W, word0, sweep, key, reverse, st);
     if (c.it <= 8 && c.itx <= 6) return launch<1, 8, 6, WIDE, W1, SG_MINB8>(d, c, W, word0, sweep, key, reverse, st);
     sg_set_error("k_vb_sweep: the slice budget of the class exceeds the kernels'");
