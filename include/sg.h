@@ -217,7 +217,7 @@ void sg_host_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t
  * every bond state sigma_i ^ sigma_j ^ kappa_ij, hence every output, unchanged.  The other entries ("X") keep a word.
  * Slices: every class is cut greedily, in position order, into runs of at most 32 sites with at most 32*it entries of
  * which at most 32*itx are X entries; (it, itx) is chosen per class, from the class's degrees, among the budgets the
- * kernels are compiled for: for odd n_words (6,4) if its cut needs at most 5 % more slices than that of (8,6), else
+ * kernels are compiled for: for odd n_words (6,4) if its cut needs at most 30 % more slices than that of (8,6), else
  * (8,6); (4,3) for n_words = 2 mod 4; (4,2) for n_words = 0 mod 4.  Inside a class every window of 4096 sites is
  * stably sorted by (demand, shape): demand 0 = a neighbour in a class of fewer than N/32 sites, 1 = fewer than N/8,
  * 2 = neither; shape 0 = at most 2 X and 2 T entries, 1 = at most 4 and 4, 2 = longer rows.  hdr[g] = 4 uint32: first

@@ -314,9 +314,12 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t 
         if (par[i] != SG_NONE) { g.tpar[p] = g.pos[par[i]]; g.teid[p] = par_e[i]; }
     }
     // per-class entry budgets (sg_internal.h): the smallest budget the kernels are compiled for whose greedy cut needs at
-    // most 5 % more slices than the largest budget's (measured: fewer, fuller slices beat shorter unrolled loops)
+    // most 30 % more slices than the largest budget's (measured: the small budget's 12 resident CTAs per SM beat the large
+    // budget's fuller slices up to there)
     // (SG_VB_IT=<it> forces one budget for all classes: a measurement knob; outputs are identical)
     const char *it_env = std::getenv("SG_VB_IT");
+    const char *slack_env = std::getenv("SG_VB_SLACK");                     // measurement knob: the percentage above
+    const uint64_t slack_pct = slack_env ? (uint64_t)std::atoi(slack_env) : 130;
     auto count_slices = [&](uint32_t k, VBBudget bud) {
         uint64_t ns = 0, p = g.cls[k].pos0;
         const uint64_t pend = p + g.cls[k].n;
@@ -340,7 +343,7 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t 
             best = SG_VB_BUDGETS_G1[NB - 1];
             const uint64_t fewest = count_slices(k, best);
             for (size_t b = 0; b + 1 < NB; ++b)
-                if (count_slices(k, SG_VB_BUDGETS_G1[b]) * 100 <= fewest * 105) { best = SG_VB_BUDGETS_G1[b]; break; }
+                if (count_slices(k, SG_VB_BUDGETS_G1[b]) * 100 <= fewest * slack_pct) { best = SG_VB_BUDGETS_G1[b]; break; }
             if (it_env)
                 for (const VBBudget bud : SG_VB_BUDGETS_G1)
                     if ((uint32_t)std::atoi(it_env) == bud.it) best = bud;

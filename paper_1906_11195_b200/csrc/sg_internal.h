@@ -35,7 +35,7 @@ Philox4 sg_philox_host(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint3
 // slice almost always share one.
 // A class is cut into slices: runs of at most 32 consecutive positions with at most capE = 32*it entries, of which at
 // most capX = 32*itx X entries (it, itx: per class, the smallest budget the kernels are compiled for that needs at most
-// 5 % more slices than the largest one; a single site always fits).  A slice is one warp's work:
+// 30 % more slices than the largest one; a single site always fits).  A slice is one warp's work:
 //   hdr[g]           = first position, first index in `col`, first index in the coupling array, and
 //                      n | nXs << 6 | nE << 16 | shape << 28  (sites, X entries, all entries of the slice, the largest
 //                      shape of its sites);

@@ -183,8 +183,18 @@ int sgk_xor_popcount_multi(const uint64_t *a, const uint64_t *const *b, uint32_t
         return SG_OK;
     }
     const uint64_t total = n_sites * W;
+    // a grid-stride kernel: exactly the CTAs that are resident at once (one wave), or fewer for small inputs
+    static int per_sm[2] = {0, 0}, n_sm = 0;
+    if (n_sm == 0) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[0], k_xor_popcount_multi<2>, 256, 0);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[1], k_xor_popcount_multi<3>, 256, 0);
+    }
     uint64_t blocks = (total + 32 * 8 * 16 - 1) / (32 * 8 * 16);
-    if (blocks > 148 * 4) blocks = 148 * 4;
+    const uint64_t wave = (uint64_t)n_sm * (uint64_t)std::max(1, per_sm[n == 2 ? 0 : 1]);
+    if (blocks > wave) blocks = wave;
     if (blocks < 1) blocks = 1;
     auto cc = [&](uint32_t s) { return (unsigned long long *)counts[s < n ? s : 0]; };
     auto bb = [&](uint32_t s) { return b[s < n ? s : 0]; };

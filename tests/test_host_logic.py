@@ -195,7 +195,7 @@ def test_host_generator_matches_oracle_and_layout_is_consistent(sg, oracle_mod, 
     assert np.all(seen_edges[~is_tree] == 2) and np.all(seen_edges[is_tree] == 0)
     assert g["entries"] == 2 * g["M"] and g["nJ"] == 2 * int((~is_tree).sum())
     # slices: greedy cut of every class into runs of <= 32 sites within the class's budgets (32*it entries, 32*itx X
-    # entries), never across classes; the budget is the first of include/sg.h's list within 5 % of the last one's slice count
+    # entries), never across classes; the budget is the first of include/sg.h's list within 30 % of the last one's slice count
     def cut(k, it, itx):
         runs = []
         p, pend = int(g["class_pos0"][k]), int(g["class_pos0"][k]) + int(g["class_n"][k])
@@ -214,7 +214,7 @@ def test_host_generator_matches_oracle_and_layout_is_consistent(sg, oracle_mod, 
     s_ = 0
     for k in range(K):
         assert int(g["class_slice0"][k]) == s_
-        best = next(b_ for b_ in budgets if 100 * len(cut(k, *b_)) <= 105 * len(cut(k, *budgets[-1])))
+        best = next(b_ for b_ in budgets if 100 * len(cut(k, *b_)) <= 130 * len(cut(k, *budgets[-1])))
         assert (int(g["class_it"][k]), int(g["class_itx"][k])) == best
         for p, n, sX, sE in cut(k, *best):
             sh = max(shape(degree[orig[q]] - nT[q], nT[q]) for q in range(p, p + n))
