@@ -121,7 +121,7 @@ int sgk_xor_popcount(const uint64_t *a, const uint64_t *b, uint64_t n_sites, uin
 // :270 counts against every stored waiting time after every sweep): 8 + 8 S bytes per site-word instead of 16 S.
 // W a power of two <= 32; counts are added to S separate rows.
 template <int S>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 2)
 k_xor_popcount_multi(const uint64_t *__restrict__ a, const uint64_t *__restrict__ b0, const uint64_t *__restrict__ b1,
                      const uint64_t *__restrict__ b2, uint64_t total, uint32_t W, unsigned long long *__restrict__ c0,
                      unsigned long long *__restrict__ c1, unsigned long long *__restrict__ c2)
@@ -138,7 +138,7 @@ k_xor_popcount_multi(const uint64_t *__restrict__ a, const uint64_t *__restrict_
     const uint64_t pol_stream = policy_evict_first();
     const uint64_t nchunks = (total + 31) / 32;
     uint32_t pending = 0;
-    constexpr int U = 2;
+    constexpr int U = 4;                       // chunks per iteration: (1 + S) * U loads in flight per thread
     for (uint64_t ch = warp; ch < nchunks; ch += (uint64_t)U * nwarps) {
         uint64_t x[U], y[S][U];
 #pragma unroll
@@ -153,10 +153,27 @@ k_xor_popcount_multi(const uint64_t *__restrict__ a, const uint64_t *__restrict_
                 for (int s = 0; s < S; ++s) y[s][u] = ld_stream_u64(b[s] + q, pol_stream);
             }
         }
+        // four one-bit numbers per lane into the counter: two carry-save adders into plane 0, one into plane 1,
+        // then the carry ripples from plane 2
 #pragma unroll
-        for (int s = 0; s < S; ++s)
+        for (int s = 0; s < S; ++s) {
+            const uint64_t d0 = x[0] ^ y[s][0], d1 = x[1] ^ y[s][1], d2 = x[2] ^ y[s][2], d3 = x[3] ^ y[s][3];
+            uint64_t ones = acc[s][0];
+            const uint64_t ta = maj64(ones, d0, d1);
+            ones ^= d0 ^ d1;
+            const uint64_t tb = maj64(ones, d2, d3);
+            ones ^= d2 ^ d3;
+            acc[s][0] = ones;
+            const uint64_t twos = acc[s][1];
+            uint64_t carry = maj64(twos, ta, tb);
+            acc[s][1] = twos ^ ta ^ tb;
 #pragma unroll
-            for (int u = 0; u < U; ++u) vc_add_bit<P, PT>(acc[s], x[u] ^ y[s][u]);
+            for (int p = 2; p < P; ++p) {
+                const uint64_t t = acc[s][p] & carry;
+                acc[s][p] ^= carry;
+                carry = t;
+            }
+        }
         pending += U;
         if (pending + U > (1u << P) - 1u) {
 #pragma unroll

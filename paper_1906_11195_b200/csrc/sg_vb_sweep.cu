@@ -376,18 +376,24 @@ __global__ void __launch_bounds__(SG_BT, MINB) k_vb_sweep(const __grid_constant_
 // counts[w*64+b] += sum over all sites of u_i (unsatisfied incident bonds of lane w*64+b) = 2 U_l; E_l = 2 U_l - M.
 // One launch over every slice of the instance; grid.y = word; a warp takes UNSAT_ROWS consecutive slices and keeps its
 // per-lane totals in vertical counters, then shared memory, then one atomicAdd per lane and CTA.
-constexpr uint32_t UNSAT_ROWS = 4;
+#ifndef SG_UNSAT_MINB
+#define SG_UNSAT_MINB 8
+#endif
+#ifndef SG_UNSAT_ROWS
+#define SG_UNSAT_ROWS 4
+#endif
+constexpr uint32_t UNSAT_ROWS = SG_UNSAT_ROWS;
 constexpr int UNSAT_IT = 8, UNSAT_ITX = 6;      // the largest budgets of SG_VB_BUDGETS_G1: serves every class
 
-template <bool WIDE>
-__global__ void __launch_bounds__(SG_BT, 8)
+template <bool WIDE, int IT, int ITX, int MINB>
+__global__ void __launch_bounds__(SG_BT, MINB)
 k_vb_unsat(const uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, const uint32_t *__restrict__ col,
            const uint32_t *__restrict__ rp_s, const SGHdr *__restrict__ hdr, uint32_t nslices, uint32_t W,
            unsigned long long *__restrict__ counts)
 {
     using I = typename Idx<WIDE>::type;
     constexpr int PT = 5 + 2 + 5;      // u <= 31, UNSAT_ROWS additions, 5 doublings in the warp
-    __shared__ __align__(16) uint64_t s_x[WARPS][32 * UNSAT_IT];
+    __shared__ __align__(16) uint64_t s_x[WARPS][32 * IT];
     __shared__ unsigned long long s_counts[64];
     uint64_t *sx = s_x[threadIdx.x >> 5];
     if (threadIdx.x < 64) s_counts[threadIdx.x] = 0;
@@ -404,7 +410,7 @@ k_vb_unsat(const uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, co
         const uint4 t = __ldg(reinterpret_cast<const uint4 *>(hdr) + slice);
         const SGHdr h{t.x, t.y, t.z, t.w};
         const uint32_t rp = ld_stream_u32(rp_s + slice * 32u + lane, pol);
-        Streams<1, UNSAT_IT, UNSAT_ITX, WIDE> st;
+        Streams<1, IT, ITX, WIDE> st;
         st.load(col, J, h, W, w, pol);
         Vec<1> own;
         own.v[0] = 0;
@@ -538,10 +544,15 @@ int sgk_vb_unsat(const VBDevice &d, uint64_t N, uint64_t nJ, uint32_t W, uint64_
     const bool wide = force_wide() || N * W >= (1ull << 32) || nJ * W >= (1ull << 32);
     const uint64_t warps = (nslices + UNSAT_ROWS - 1) / UNSAT_ROWS;
     dim3 grid((unsigned)((warps + WARPS - 1) / WARPS), W);
-    if (wide)
-        k_vb_unsat<true><<<grid, SG_BT, 0, st>>>(d.spin, d.J, d.col, d.rp_s, d.hdr, (uint32_t)nslices, W, (unsigned long long *)counts);
-    else
-        k_vb_unsat<false><<<grid, SG_BT, 0, st>>>(d.spin, d.J, d.col, d.rp_s, d.hdr, (uint32_t)nslices, W, (unsigned long long *)counts);
+    // the instantiation for the instance's largest per-class budget
+    const bool small = d.it_max <= 6 && d.itx_max <= 4;
+    auto go = [&](auto kern) {
+        static bool carved = false;     // per instantiation (the lambda is instantiated once per kernel)
+        if (!carved) { cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 28); carved = true; }
+        kern<<<grid, SG_BT, 0, st>>>(d.spin, d.J, d.col, d.rp_s, d.hdr, (uint32_t)nslices, W, (unsigned long long *)counts);
+    };
+    if (wide) { if (small) go(k_vb_unsat<true, 6, 4, SG_UNSAT_MINB>); else go(k_vb_unsat<true, UNSAT_IT, UNSAT_ITX, 7>); }
+    else { if (small) go(k_vb_unsat<false, 6, 4, SG_UNSAT_MINB>); else go(k_vb_unsat<false, UNSAT_IT, UNSAT_ITX, 7>); }
     sgk_count_launch();
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { sg_set_error(std::string("k_vb_unsat launch failed: ") + cudaGetErrorString(e)); return SG_ECUDA; }
