@@ -36,7 +36,7 @@ void sgk_count_launch();
 
 namespace {
 
-constexpr int SK_THREADS = 256;
+constexpr int SK_THREADS = 288;      // warp 0 decides, the other eight apply
 constexpr uint32_t SK_CLONE_STRIDE = 1u << 20;
 
 __host__ __device__ inline uint32_t sk_nw32(uint64_t N) { return (uint32_t)((N + 31) / 32); }
@@ -124,6 +124,10 @@ __global__ void __launch_bounds__(256) k_sk_init_spins(uint32_t *__restrict__ sb
     sbits[(l0 + 32) * NW32 + wq] = mine1;
 }
 
+// named barriers of the sweep kernel (producer / consumer between the deciding warp and the others)
+__device__ __forceinline__ void sk_bar_sync(uint32_t id) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(SK_THREADS) : "memory"); }
+__device__ __forceinline__ void sk_bar_arrive(uint32_t id) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(SK_THREADS) : "memory"); }
+
 // ---------------------------------------------------------------------------------------- the sweep
 // dynamic shared memory: int16 Hs[32 * nw32p] (transposed: field of site j at (j%32)*nw32p + j/32),
 //                        u32 rs[32 * NW32] (this sweep's uniforms), u32 sp[NW32] (spin bits), u32 ctl[4]
@@ -157,12 +161,21 @@ k_sk_sweep(const uint32_t *__restrict__ rows, int16_t *__restrict__ Hg, uint32_t
             philox4x32_10(i, w >> 2, (uint32_t)t, (uint32_t)(t >> 32), k0, k1, x);
             rs[i] = (w & 2u) ? ((w & 1u) ? x[3] : x[2]) : ((w & 1u) ? x[1] : x[0]);
         }
-        uint32_t diag = 0;   // warp 0: lane l holds row (32 b + l), word b  (the 32x32 diagonal block)
-        if (warp == 0 && lane < N) diag = myrows[(uint64_t)lane * NW32 + 0];
-        __syncthreads();
-
-        for (uint32_t b = 0; b < NW32; ++b) {
-            if (warp == 0) {
+        // Two roles, one batch apart.  Warp 0 (the decider) visits the 32 sites of batch b in order, then adds the batch's
+        // flips to the 32 fields of batch b + 1 (the only fields its next decision reads) and publishes the flips; warps
+        // 1-7 (the workers) add them to every other field while the decider is already at batch b + 1.
+        //   full[b & 1]: the decider has published batch b          (decider arrives, workers wait)
+        //   done[b & 1]: the workers have applied batch b           (workers arrive, decider waits before it touches the
+        //                fields of batch b + 2, which the workers of batch b also write)
+        // decider: lane l prefetches, of row 32 b + l, word b (the 32 x 32 diagonal block) and word b + 1 (towards the next batch)
+        uint32_t diag = 0, nxt = 0;
+        if (warp == 0 && lane < N) {
+            diag = myrows[(uint64_t)lane * NW32 + 0];
+            if (NW32 > 1) nxt = myrows[(uint64_t)lane * NW32 + 1];
+        }
+        __syncthreads();                                              // uniforms of this sweep are in place
+        if (warp == 0) {
+            for (uint32_t b = 0; b < NW32; ++b) {
                 const uint32_t i = 32u * b + lane;
                 const bool valid = i < N;
                 int h = Hs[lane * nw32p + b];
@@ -187,35 +200,79 @@ k_sk_sweep(const uint32_t *__restrict__ rows, int16_t *__restrict__ Hg, uint32_t
                     todo = (k == 31u) ? 0u : (0xFFFFFFFFu << (k + 1u));
                 }
                 Hs[lane * nw32p + b] = (int16_t)h;
-                if (lane == 0) { sp[b] = spw; ctl[b & 1u] = F; }   // double-buffered: warp 0 may run one batch ahead
-                // prefetch the next diagonal block while the CTA applies this batch's flips
+                if (b >= 1) sk_bar_sync(3u + ((b - 1u) & 1u));        // done[b - 1]: nobody else writes batch b + 1's fields now
                 if (b + 1 < NW32) {
-                    const uint32_t inext = 32u * (b + 1) + lane;
-                    diag = inext < N ? myrows[(uint64_t)inext * NW32 + (b + 1)] : 0u;
-                }
-            }
-            __syncthreads();
-            const uint32_t F = ctl[b & 1u];
-            if (F) {
-                const uint32_t spw = sp[b];
-                // each thread owns half-words of the row: item it -> word it>>1, bits 16*(it&1) .. +15
-                for (uint32_t it = tid; it < 2u * NW32; it += SK_THREADS) {
-                    const uint32_t wq = it >> 1, half = it & 1u;
-                    if (wq == b) continue;                            // diagonal block already done by warp 0
+                    int hn = Hs[lane * nw32p + b + 1];
                     uint32_t Fl = F;
                     while (Fl) {
                         const uint32_t k = __ffs(Fl) - 1u;
                         Fl &= Fl - 1u;
                         const int snew2 = ((spw >> k) & 1u) ? -2 : 2;
-                        const uint32_t rw = myrows[(uint64_t)(32u * b + k) * NW32 + wq] >> (16u * half);
-                        int16_t *hp = Hs + (16u * half) * nw32p + wq;
-#pragma unroll
-                        for (int q = 0; q < 16; ++q) hp[q * nw32p] += (int16_t)(((rw >> q) & 1u) ? -snew2 : snew2);
+                        const uint32_t rw = __shfl_sync(0xFFFFFFFFu, nxt, k);
+                        hn += ((rw >> lane) & 1u) ? -snew2 : snew2;
+                    }
+                    Hs[lane * nw32p + b + 1] = (int16_t)hn;
+                }
+                if (lane == 0) { sp[b] = spw; ctl[b & 1u] = F; }
+                __threadfence_block();
+                sk_bar_arrive(1u + (b & 1u));                         // full[b]
+                if (b + 1 < NW32) {                                   // prefetch for the next batch
+                    const uint32_t inext = 32u * (b + 1) + lane;
+                    diag = 0; nxt = 0;
+                    if (inext < N) {
+                        diag = myrows[(uint64_t)inext * NW32 + (b + 1)];
+                        if (b + 2 < NW32) nxt = myrows[(uint64_t)inext * NW32 + (b + 2)];
                     }
                 }
-                __syncthreads();
+            }
+            sk_bar_sync(3u + ((NW32 - 1u) & 1u));                     // done[last]
+        } else {
+            const uint32_t wtid = tid - 32u;
+            for (uint32_t b = 0; b < NW32; ++b) {
+                sk_bar_sync(1u + (b & 1u));                           // full[b]
+                const uint32_t F = ctl[b & 1u];
+                if (F) {
+                    const uint32_t spw = sp[b];
+                    // each thread owns half-words of the row: item it -> word it>>1, bits 16*(it&1) .. +15
+                    for (uint32_t it = wtid; it < 2u * NW32; it += SK_THREADS - 32u) {
+                        const uint32_t wq = it >> 1, half = it & 1u;
+                        if (wq == b || wq == b + 1u) continue;        // done by the decider
+                        int16_t *hp = Hs + (16u * half) * nw32p + wq;
+                        uint32_t Fl = F;
+                        while (Fl) {
+                            // up to four flips at a time: their row words are read together (independent loads), then added
+                            uint32_t kk[4], rw[4];
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                kk[u] = 32u;
+                                rw[u] = 0;
+                                if (Fl) {
+                                    kk[u] = __ffs(Fl) - 1u;
+                                    Fl &= Fl - 1u;
+                                    rw[u] = myrows[(uint64_t)(32u * b + kk[u]) * NW32 + wq] >> (16u * half);
+                                }
+                            }
+                            int d[16];
+#pragma unroll
+                            for (int q = 0; q < 16; ++q) d[q] = 0;
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                if (kk[u] < 32u) {
+                                    const int snew2 = ((spw >> kk[u]) & 1u) ? -2 : 2;
+#pragma unroll
+                                    for (int q = 0; q < 16; ++q) d[q] += ((rw[u] >> q) & 1u) ? -snew2 : snew2;
+                                }
+                            }
+#pragma unroll
+                            for (int q = 0; q < 16; ++q) hp[q * nw32p] += (int16_t)d[q];
+                        }
+                    }
+                }
+                __threadfence_block();
+                sk_bar_arrive(3u + (b & 1u));                         // done[b]
             }
         }
+        __syncthreads();                                              // end of the sweep: every field is up to date
     }
     __syncthreads();
     for (uint32_t j = tid; j < N; j += SK_THREADS) myH[j] = Hs[(j & 31u) * nw32p + (j >> 5)];
