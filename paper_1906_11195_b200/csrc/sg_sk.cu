@@ -17,6 +17,8 @@
 // 2 J'_ij s_i to every other field for each accepted flip i of the batch, reading row i once.
 #include <cuda_runtime.h>
 
+#include <cstdlib>
+
 #include <algorithm>
 
 #include "sg_device.cuh"
@@ -38,6 +40,7 @@ namespace {
 
 constexpr int SK_THREADS = 288;      // warp 0 decides, the other eight apply
 constexpr uint32_t SK_CLONE_STRIDE = 1u << 20;
+constexpr int SK_PRE = 8;                // uint4 a worker thread stages per batch: 256 threads * 8 * 16 B = 32 KiB = the block at N = 8192
 
 __host__ __device__ inline uint32_t sk_nw32(uint64_t N) { return (uint32_t)((N + 31) / 32); }
 // padded row length of the transposed field array in shared memory: 2 * odd, so that the 32 lanes of
@@ -134,7 +137,7 @@ __device__ __forceinline__ void sk_bar_arrive(uint32_t id) { asm volatile("bar.a
 __global__ void __launch_bounds__(SK_THREADS)
 k_sk_sweep(const uint32_t *__restrict__ rows, int16_t *__restrict__ Hg, uint32_t *__restrict__ sbits,
            const uint64_t *__restrict__ thr, uint32_t N, uint32_t NW32, uint32_t mz /* thr[m] = 0 for m >= mz */,
-           uint32_t lanes_w, uint32_t word0, uint64_t sweep0, uint32_t nsweeps, uint32_t k0, uint32_t k1)
+           uint32_t lanes_w, uint32_t word0, uint64_t sweep0, uint32_t nsweeps, uint32_t k0, uint32_t k1, uint32_t stage_off /* 0: rows not staged */)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const uint32_t nw32p = sk_nw32p(NW32);
@@ -142,6 +145,8 @@ k_sk_sweep(const uint32_t *__restrict__ rows, int16_t *__restrict__ Hg, uint32_t
     uint32_t *rs = reinterpret_cast<uint32_t *>(smem_raw + ((32u * nw32p * 2u + 15u) & ~15u));
     uint32_t *sp = rs + 32u * NW32;
     volatile uint32_t *ctl = sp + NW32;
+    const bool staged = stage_off != 0;
+    uint4 *rowbuf = reinterpret_cast<uint4 *>(smem_raw + stage_off);      // two buffers of 32 * NW32 words (8 * NW32 uint4)
 
     const uint32_t lane_g = blockIdx.x;
     const uint32_t w = word0 + ((lane_g % lanes_w) >> 6) + (lane_g / lanes_w) * SK_CLONE_STRIDE;   // virtual word of the uniforms
@@ -228,9 +233,26 @@ k_sk_sweep(const uint32_t *__restrict__ rows, int16_t *__restrict__ Hg, uint32_t
             sk_bar_sync(3u + ((NW32 - 1u) & 1u));                     // done[last]
         } else {
             const uint32_t wtid = tid - 32u;
+            constexpr uint32_t NWK = SK_THREADS - 32u;                // worker threads
+            const uint32_t blk4 = 8u * NW32;                          // uint4 per staged block (32 full rows: N % 128 == 0)
+            if (staged) {                                             // batch 0's rows; the full[0] barrier below publishes them
+                const uint4 *g4 = reinterpret_cast<const uint4 *>(myrows);
+                for (uint32_t q = wtid; q < blk4; q += NWK) rowbuf[q] = __ldg(g4 + q);
+            }
             for (uint32_t b = 0; b < NW32; ++b) {
-                sk_bar_sync(1u + (b & 1u));                           // full[b]
+                sk_bar_sync(1u + (b & 1u));                           // full[b]: also, every worker is past batch b - 1
                 const uint32_t F = ctl[b & 1u];
+                // the next batch's rows: loads issued now, stored to the other buffer after this batch's work
+                uint4 pre[SK_PRE];
+                const bool more = staged && b + 1 < NW32;
+                if (more) {
+                    const uint4 *g4 = reinterpret_cast<const uint4 *>(myrows + (uint64_t)32u * (b + 1) * NW32);
+#pragma unroll
+                    for (int u = 0; u < SK_PRE; ++u)
+                        if (wtid + u * NWK < blk4) pre[u] = __ldg(g4 + wtid + u * NWK);
+                }
+                const uint32_t *grow = myrows + (uint64_t)32u * b * NW32;                                    // rows of this batch, global
+                const uint32_t *srow = reinterpret_cast<const uint32_t *>(rowbuf + (b & 1u) * blk4);          // ... and staged
                 if (F) {
                     const uint32_t spw = sp[b];
                     // each thread owns half-words of the row: item it -> word it>>1, bits 16*(it&1) .. +15
@@ -249,7 +271,7 @@ k_sk_sweep(const uint32_t *__restrict__ rows, int16_t *__restrict__ Hg, uint32_t
                                 if (Fl) {
                                     kk[u] = __ffs(Fl) - 1u;
                                     Fl &= Fl - 1u;
-                                    rw[u] = myrows[(uint64_t)(32u * b + kk[u]) * NW32 + wq] >> (16u * half);
+                                    rw[u] = (staged ? srow[kk[u] * NW32 + wq] : __ldg(grow + kk[u] * NW32 + wq)) >> (16u * half);
                                 }
                             }
                             int d[16];
@@ -267,6 +289,11 @@ k_sk_sweep(const uint32_t *__restrict__ rows, int16_t *__restrict__ Hg, uint32_t
                             for (int q = 0; q < 16; ++q) hp[q * nw32p] += (int16_t)d[q];
                         }
                     }
+                }
+                if (more) {
+#pragma unroll
+                    for (int u = 0; u < SK_PRE; ++u)
+                        if (wtid + u * NWK < blk4) rowbuf[((b + 1u) & 1u) * blk4 + wtid + u * NWK] = pre[u];
                 }
                 __threadfence_block();
                 sk_bar_arrive(3u + (b & 1u));                         // done[b]
@@ -320,11 +347,20 @@ __global__ void __launch_bounds__(256) k_sk_correlation(const uint32_t *__restri
     }
 }
 
-size_t sk_smem_bytes(uint32_t NW32)
+// The 32 coupling rows of a batch are one contiguous block of 128 * NW32 bytes; for N <= 8192 (and N a multiple of 128, so
+// that the block is a whole number of 16-byte units) two such blocks fit in shared memory: the workers copy the next
+// batch's block in while they apply the current batch (SG_SK_STAGE=0 switches that off: a measurement knob).
+bool sk_staged(uint32_t NW32)
+{
+    static const bool off = std::getenv("SG_SK_STAGE") && std::getenv("SG_SK_STAGE")[0] == '0';
+    return !off && NW32 % 4u == 0 && NW32 <= 256u;
+}
+size_t sk_smem_base(uint32_t NW32)
 {
     const uint32_t nw32p = sk_nw32p(NW32);
-    return ((32u * nw32p * 2u + 15u) & ~15u) + 4u * (32u * NW32 + NW32 + 4u);
+    return (((32u * nw32p * 2u + 15u) & ~15u) + 4u * (32u * NW32 + NW32 + 4u) + 15u) & ~(size_t)15u;
 }
+size_t sk_smem_bytes(uint32_t NW32) { return sk_smem_base(NW32) + (sk_staged(NW32) ? 2u * 128u * NW32 : 0u); }
 
 }  // namespace
 
@@ -381,7 +417,8 @@ int sg_sk_sweep_impl(sg_sim *h, uint64_t n)
     while (n) {
         const uint32_t chunk = (uint32_t)std::min<uint64_t>(n, 1u << 20);
         k_sk_sweep<<<(unsigned)h->lanes, SK_THREADS, smem, st>>>(h->sk.rows, h->sk.H, (uint32_t *)h->sk.spin, h->sk.thr, (uint32_t)h->N, NW32,
-                                                                 h->sk.nthr_nz, 64u * h->W, h->word0, h->sweep, chunk, h->key.k0, h->key.k1);
+                                                                 h->sk.nthr_nz, 64u * h->W, h->word0, h->sweep, chunk, h->key.k0, h->key.k1,
+                                                                 sk_staged(NW32) ? (uint32_t)sk_smem_base(NW32) : 0u);
         SK_LAUNCH_CHECK();
         h->sweep += chunk;
         n -= chunk;
