@@ -262,12 +262,13 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t 
     auto shape_of = [&](uint32_t i) { return sg_vb_shape((uint32_t)(g.row_ptr[i + 1] - g.row_ptr[i]) - nT[i], nT[i]); };
     const char *dem_env = std::getenv("SG_VB_DEMAND");                      // measurement knob: 0 = sort by shape only
     const bool use_demand = !(dem_env && !std::strcmp(dem_env, "0"));
+    const uint64_t demand2_div = (dem_env && !std::strcmp(dem_env, "2")) ? (1ull << 40) : 4;      // "2": only the two smaller brackets
     auto bucket_of = [&](uint32_t i) {
-        uint32_t demand = 2;
+        uint32_t demand = 3;
         if (use_demand)
             for (uint64_t a = g.row_ptr[i]; a < g.row_ptr[i + 1]; ++a) {
                 const uint64_t nk = ccount[g.colour[g.adj[a]]];
-                demand = std::min(demand, nk * 32 < N ? 0u : nk * 8 < N ? 1u : 2u);
+                demand = std::min(demand, nk * 32 < N ? 0u : nk * 8 < N ? 1u : nk * demand2_div < N ? 2u : 3u);
             }
         return demand * 3 + shape_of(i);
     };
@@ -287,8 +288,9 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t 
         else for (uint64_t q = 0; q < N; ++q) g.orig[fill[g.colour[bfs[q]]]++] = bfs[q];
         // Buckets: every window of `win` consecutive sites of a class (in the order above) is stably sorted by
         // (demand, shape).  demand: 0 = the site has a neighbour in a class of fewer than N/32 sites, 1 = in a class
-        // of fewer than N/8 sites, 2 = neither: the small classes gather from few sites, and with those packed
-        // together their gathers use whole 128-byte lines instead of one word per line.  shape (sg_vb_shape): 0 = at
+        // of fewer than N/8 sites, 2 = of fewer than N/4 sites, 3 = none of these: the smaller classes gather from a
+        // part of the sites only, and with those packed together their gathers use whole 128-byte lines and a smaller
+        // part of L2.  shape (sg_vb_shape): 0 = at
         // most 2 X and 2 T entries, 1 = at most 4 and 4, 2 = longer rows: almost every slice then holds sites of one
         // shape and the kernels run the count that fits it.  The breadth-first order survives inside each run.
         if (win > 1) {
@@ -296,9 +298,9 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t 
             for (uint32_t k = 0; k < K; ++k)
                 for (uint64_t a = g.cls[k].pos0, end = a + g.cls[k].n; a < end; a += win) {
                     const uint64_t len = std::min<uint64_t>(win, end - a);
-                    uint64_t at[10] = {0};
+                    uint64_t at[13] = {0};
                     for (uint64_t q = 0; q < len; ++q) at[bucket_of(g.orig[a + q]) + 1]++;
-                    for (int b = 0; b < 9; ++b) at[b + 1] += at[b];
+                    for (int b = 0; b < 12; ++b) at[b + 1] += at[b];
                     for (uint64_t q = 0; q < len; ++q) tmp[at[bucket_of(g.orig[a + q])]++] = g.orig[a + q];
                     std::copy(tmp.begin(), tmp.begin() + len, g.orig.begin() + a);
                 }

@@ -144,12 +144,13 @@ def test_host_generator_matches_oracle_and_layout_is_consistent(sg, oracle_mod, 
     degree = np.bincount(e.ravel().astype(np.int64), minlength=N)
     rows, order, par, par_e = _bfs_forest(N, e)
     # positions: class-major; inside a class breadth-first order, every window of 4096 sites stably sorted by
-    # (demand, shape); demand 0: a neighbour in a class of fewer than N/32 sites, 1: fewer than N/8, 2: neither;
+    # (demand, shape); demand 0: a neighbour in a class of fewer than N/32 sites, 1: fewer than N/8, 2: fewer than N/4, 3: none;
     # shape 0: at most 2 X and 2 T entries, 1: at most 4 and 4, 2: longer rows (T = forest edges, X = the others)
     csize = np.bincount(colour, minlength=K)
 
     def demand(i):
-        return min([2] + [0 if 32 * csize[colour[v_]] < N else 1 if 8 * csize[colour[v_]] < N else 2 for v_, _ in rows[i]])
+        return min([3] + [0 if 32 * csize[colour[v_]] < N else 1 if 8 * csize[colour[v_]] < N else 2 if 4 * csize[colour[v_]] < N else 3
+                          for v_, _ in rows[i]])
     nT_lab = np.zeros(N, dtype=np.int64)
     for i in range(N):
         if par[i] >= 0:
