@@ -53,6 +53,8 @@ enum { SG_OK = 0, SG_EINVAL = -1, SG_ENOMEM = -2, SG_ECUDA = -3, SG_ESLOT = -4 }
  *   seed    Philox key.  (model, N, c, T, seed, n_words) determine every bit of every output.
  *   n_words 64-bit words per site, 1 <= n_words <= 65535; lane l = 64*w + b is bit b of word w.
  * Spins start uniformly random, sweep counter = 0.
+ * The handle belongs to the CUDA device that is current at this call; sg_sweep, sg_snapshot, sg_correlation, sg_energy
+ * and sg_corr_accumulate return SG_EINVAL when another device is current.  Work is enqueued on torch's current stream.
  * Returns NULL on failure (bad argument, no CUDA device, out of memory).
  */
 sg_sim *sg_create(int model, uint64_t N, double c, double T, uint64_t seed, uint32_t n_words);

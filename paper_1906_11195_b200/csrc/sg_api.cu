@@ -22,6 +22,18 @@ extern "C" uint64_t sg_kernel_launches(void) { return sgk_launch_count(); }
 
 namespace {
 
+// A handle's buffers live on the device that was current at sg_create; launching on another device (after a
+// torch.cuda.set_device, say) would be an error that CUDA reports late and far away.
+bool on_own_device(const sg_sim *h, const char *who)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != h->device) {
+        sg_set_error(std::string(who) + ": the current CUDA device is not the one the handle was created on");
+        return false;
+    }
+    return true;
+}
+
 void destroy_impl(sg_sim *h)
 {
     if (!h) return;
@@ -123,6 +135,7 @@ extern "C" sg_sim *sg_create_opt(int model, uint64_t N, double c, double T, uint
     h->word0 = o.word0; h->clones = o.n_clones; h->aligned = o.aligned_start != 0;
     h->lanes = 64ull * n_words * o.n_clones;
     h->key = SGSeed{(uint32_t)seed, (uint32_t)(seed >> 32)};
+    cudaGetDevice(&h->device);
     int rc;
     try {
         rc = (model == SG_MODEL_VB) ? create_vb(h) : sg_sk_create_impl(h);
@@ -143,6 +156,7 @@ extern "C" void sg_destroy(sg_sim *h) { destroy_impl(h); }
 extern "C" int sg_sweep(sg_sim *h, uint64_t n)
 {
     if (!h) { sg_set_error("sg_sweep: null handle"); return SG_EINVAL; }
+    if (!on_own_device(h, "sg_sweep")) return SG_EINVAL;
     if (h->sweep + n >= (1ull << 56)) { sg_set_error("sg_sweep: sweep counter would exceed 2^56"); return SG_EINVAL; }
     if (h->model == SG_MODEL_SK) return sg_sk_sweep_impl(h, n);
     cudaStream_t st = sgx_stream();
@@ -234,6 +248,7 @@ static uint64_t *current_config(sg_sim *h) { return h->model == SG_MODEL_VB ? h-
 extern "C" int sg_snapshot(sg_sim *h, uint32_t slot)
 {
     if (!h) { sg_set_error("sg_snapshot: null handle"); return SG_EINVAL; }
+    if (!on_own_device(h, "sg_snapshot")) return SG_EINVAL;
     if (slot >= SG_MAX_SLOTS) { sg_set_error("sg_snapshot: slot out of range"); return SG_EINVAL; }
     if (!h->slot[slot]) {
         h->slot[slot] = dev_alloc<uint64_t>(h, h->spin_words);
@@ -248,6 +263,7 @@ extern "C" int sg_snapshot(sg_sim *h, uint32_t slot)
 extern "C" int sg_correlation(sg_sim *h, uint32_t slot, uint64_t *out_counts)
 {
     if (!h || !out_counts) { sg_set_error("sg_correlation: null argument"); return SG_EINVAL; }
+    if (!on_own_device(h, "sg_correlation")) return SG_EINVAL;
     if (slot >= SG_MAX_SLOTS) { sg_set_error("sg_correlation: slot out of range"); return SG_EINVAL; }
     if (!h->slot[slot]) { sg_set_error("sg_correlation: slot was never written"); return SG_ESLOT; }
     cudaStream_t st = sgx_stream();
@@ -282,6 +298,7 @@ extern "C" int sg_corr_configure(sg_sim *h, uint32_t nbins)
 extern "C" int sg_corr_accumulate(sg_sim *h, uint32_t n, const uint32_t *slots, const uint32_t *bins)
 {
     if (!h || (n && (!slots || !bins))) { sg_set_error("sg_corr_accumulate: null argument"); return SG_EINVAL; }
+    if (!on_own_device(h, "sg_corr_accumulate")) return SG_EINVAL;
     if (!h->corr_acc) { sg_set_error("sg_corr_accumulate: call sg_corr_configure first"); return SG_EINVAL; }
     for (uint32_t k = 0; k < n; ++k) {
         if (slots[k] >= SG_MAX_SLOTS || bins[k] >= h->corr_bins) { sg_set_error("sg_corr_accumulate: slot or bin out of range"); return SG_EINVAL; }
@@ -323,6 +340,7 @@ extern "C" int sg_corr_fetch(sg_sim *h, uint32_t bin0, uint32_t nbins, uint64_t 
 extern "C" int sg_energy(sg_sim *h, int64_t *out)
 {
     if (!h || !out) { sg_set_error("sg_energy: null argument"); return SG_EINVAL; }
+    if (!on_own_device(h, "sg_energy")) return SG_EINVAL;
     if (h->model == SG_MODEL_SK) return sg_sk_energy_impl(h, out);
     cudaStream_t st = sgx_stream();
     const uint64_t lanes = h->lanes;

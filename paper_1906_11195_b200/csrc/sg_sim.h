@@ -18,6 +18,7 @@ struct sg_sim {
     double c = 0, T = 0;
     uint64_t seed = 0;
     uint64_t sweep = 0;
+    int device = -1;                         // the CUDA device the handle was created on: every call checks it
     SGSeed key{0, 0};
     // VB
     VBHostGraph g;
