@@ -307,7 +307,7 @@ def run_ours(args):
                                 else f"{args.model.upper()} degree 4 N=2^{args.log2n} W={W} T={args.T} seed=1+rank (the paper's ensemble, PAPER.md:75, :260; not the headline workload)" if args.model in ("rrbg", "rrg")
                                 else f"SK N=2^{args.log2n} W={W} T={args.T} seed=1+rank (BASELINE.json configs[3]; dependency-latency bound, roofline fields not meaningful)"),
                    "step": f"sg_sweep({SWEEPS_PER_STEP}) + sg_snapshot + sg_correlation + sg_energy",
-                   "l2": "inputs larger than L2: every sweep streams 777 MiB of couplings+indices+labels and reads/writes the 128 MiB spin array (L2 126 MiB); no flush needed",
+                   "l2": "inputs larger than L2: every sweep streams 660 MiB of couplings+indices+labels+headers and reads/writes the 128 MiB spin array (L2 126 MiB); no flush needed",
                    "parallelism": ("one instance sharded by site: per-class NCCL exchange of the updated slices" if site else
                                    "replicas sharded by sample word, no data-path collective") if world > 1 else "single GPU",
                    "create_s": round(create_s, 2)},

@@ -471,10 +471,11 @@ int launch(const VBDevice &d, const VBClass &c, uint32_t W, uint32_t word0, uint
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)((jobs + WARPS - 1) / WARPS));
     cfg.blockDim = dim3(SG_BT);
-    // Shared-memory carve-out: 64 KiB (28 % of 228), enough for 10 resident CTAs of the common instantiations, so that
-    // 192 KiB stay L1.  The gathers keep thousands of lines in flight per SM and L1 is where they land: with the
-    // driver's default choice (about 100 KiB of shared memory) the sweep is 3.5 % slower, with a 228 KiB carve-out
-    // 2.5 x slower; 32 KiB (6 CTAs) is 5 % slower (profiles/r02_sweep.md).  SG_VB_CARVEOUT=<percent>: measurement knob.
+    // Shared-memory carve-out: a preference of 28 % makes the driver configure 100 KiB of shared memory -- the smallest
+    // size that holds the 12 CTAs (7 KiB each with the system's 1 KiB) the register file admits -- and leaves 156 KiB L1.
+    // The gathers keep thousands of lines in flight per SM and L1 is where they land: the driver's own default is
+    // 3.5 % slower, 44 % (132 KiB) 5 % slower, 100 % (228 KiB) 2.5 x slower; 14-24 % (64 KiB, 9 CTAs) is 5 % slower
+    // too (profiles/r02_sweep.md).  SG_VB_CARVEOUT=<percent>: measurement knob.
     static const int carve_pct = std::getenv("SG_VB_CARVEOUT") ? std::atoi(std::getenv("SG_VB_CARVEOUT")) : 28;
     static bool carved = false;             // per instantiation
     if (!carved) {
