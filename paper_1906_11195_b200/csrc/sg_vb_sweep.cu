@@ -476,11 +476,12 @@ int launch(const VBDevice &d, const VBClass &c, uint32_t W, uint32_t word0, uint
     // The gathers keep thousands of lines in flight per SM and L1 is where they land: the driver's own default is
     // 3.5 % slower, 44 % (132 KiB) 5 % slower, 100 % (228 KiB) 2.5 x slower; 14-24 % (64 KiB, 9 CTAs) is 5 % slower
     // too (profiles/r02_sweep.md).  SG_VB_CARVEOUT=<percent>: measurement knob.
-    static const int carve_pct = std::getenv("SG_VB_CARVEOUT") ? std::atoi(std::getenv("SG_VB_CARVEOUT")) : 28;
-    static bool carved = false;             // per instantiation
-    if (!carved) {
+    const char *carve_env = std::getenv("SG_VB_CARVEOUT");      // read at every launch, like the other knobs: tests switch them
+    const int carve_pct = carve_env ? std::atoi(carve_env) : 28;
+    static int carved = -1;                 // per instantiation: the preference that is in force
+    if (carved != carve_pct) {
         cudaFuncSetAttribute(k_vb_sweep<G, IT, ITX, WIDE, W1, MINB>, cudaFuncAttributePreferredSharedMemoryCarveout, carve_pct);
-        carved = true;
+        carved = carve_pct;
     }
     cfg.dynamicSmemBytes = 0;
     cfg.stream = st;
@@ -488,7 +489,7 @@ int launch(const VBDevice &d, const VBClass &c, uint32_t W, uint32_t word0, uint
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see griddep_wait() in the kernel
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    static const bool no_pdl = std::getenv("SG_NO_PDL") != nullptr;   // measurement knob
+    const bool no_pdl = std::getenv("SG_NO_PDL") != nullptr;   // measurement knob
     cfg.numAttrs = no_pdl ? 0 : 1;
     const cudaError_t le = cudaLaunchKernelEx(&cfg, k_vb_sweep<G, IT, ITX, WIDE, W1, MINB>, a);
     sgk_count_launch();

@@ -219,6 +219,25 @@ def test_relabelling_does_not_change_any_output(sg, oracle_mod, monkeypatch, ord
     assert np.array_equal(g.correlation(1), o.correlation(1))
 
 
+@pytest.mark.parametrize("knob,value", [("SG_VB_IT", "6"), ("SG_VB_IT", "8"), ("SG_VB_WIN", "0"), ("SG_VB_WIN", "64"),
+                                        ("SG_VB_DEMAND", "0"), ("SG_VB_GAUGE", "0"), ("SG_VB_SLACK", "100"),
+                                        ("SG_VB_CARVEOUT", "50"), ("SG_NO_PDL", "1")])
+@pytest.mark.parametrize("N,c,T,seed,W", [(20000, 4.0, 1.0, 21, 1), (3000, 9.0, 0.6, 22, 3)])
+def test_layout_and_launch_knobs_change_no_output(sg, oracle_mod, monkeypatch, knob, value, N, c, T, seed, W):
+    """The measurement knobs of DESIGN.md section 10 choose among layouts and launch configurations (entry budget of a
+    slice, hence the kernel instantiation; window of the (demand, shape) sort; gauge fixing; shared-memory carve-out;
+    programmatic dependent launch): every one of them must leave every output bit as it is."""
+    monkeypatch.setenv(knob, value)
+    g, o = _pair(sg, oracle_mod, N, c, T, seed, W)
+    assert np.array_equal(g.couplings(), o.couplings())
+    g.snapshot(0); o.snapshot(0)
+    for _ in range(3):
+        g.sweep(2); o.sweep(2)
+        _assert_same_state(g, o)
+    assert np.array_equal(g.energy(), o.energy())
+    assert np.array_equal(g.correlation(0), o.correlation(0))
+
+
 def _lane_counts(x):
     """per-lane popcount over sites of an (N, W) uint64 array -> 64*W counts (plain numpy, no oracle, no CUDA)"""
     out = np.zeros(64 * x.shape[1], dtype=np.uint64)
