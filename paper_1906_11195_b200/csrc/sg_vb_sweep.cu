@@ -380,7 +380,7 @@ __global__ void __launch_bounds__(SG_BT, MINB) k_vb_sweep(const __grid_constant_
 #define SG_UNSAT_MINB 8
 #endif
 #ifndef SG_UNSAT_ROWS
-#define SG_UNSAT_ROWS 4
+#define SG_UNSAT_ROWS 16
 #endif
 constexpr uint32_t UNSAT_ROWS = SG_UNSAT_ROWS;
 constexpr int UNSAT_IT = 8, UNSAT_ITX = 6;      // the largest budgets of SG_VB_BUDGETS_G1: serves every class
@@ -392,7 +392,8 @@ k_vb_unsat(const uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, co
            unsigned long long *__restrict__ counts)
 {
     using I = typename Idx<WIDE>::type;
-    constexpr int PT = 5 + 2 + 5;      // u <= 31, UNSAT_ROWS additions, 5 doublings in the warp
+    constexpr int LR = UNSAT_ROWS <= 2 ? 1 : UNSAT_ROWS <= 4 ? 2 : UNSAT_ROWS <= 8 ? 3 : 4;
+    constexpr int PT = 5 + LR + 5;     // u <= 31, UNSAT_ROWS additions, 5 doublings in the warp
     __shared__ __align__(16) uint64_t s_x[WARPS][32 * IT];
     __shared__ unsigned long long s_counts[64];
     uint64_t *sx = s_x[threadIdx.x >> 5];
@@ -421,7 +422,7 @@ k_vb_unsat(const uint64_t *__restrict__ spin, const uint64_t *__restrict__ J, co
         count_unsatisfied<1>(sx, rp, own, P);
         __syncwarp();
         const uint64_t pl[5] = {P.p[0][0], P.p[1][0], P.p[2][0], P.p[3][0], P.p[4][0]};
-        vc_add_planes<5 + 2, PT, 5>(acc, pl);
+        vc_add_planes<5 + LR, PT, 5>(acc, pl);
     }
     vc_warp_flush<PT>(acc, 1, 0, s_counts);
     __syncthreads();
