@@ -228,7 +228,7 @@ void sg_host_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t
  * X entries in site order (per site by ascending position), then the T entries in site order (per site: parent first,
  * then the children by ascending position); the coupling entries follow the X order, jeid gives the edge id of each.
  * orig_s[32g + j] = label of the j-th site of slice g (0xFFFFFFFF for j >= n); rp_s[32g + j] =
- * xOff | tOff << 8 | nX << 16 | nT << 21: where the site's X / T entries start inside the slice's run (tOff >= nXs),
+ * xOff | tOff << 8 | nX << 17 | nT << 22: where the site's X / T entries start inside the slice's run (nXs <= tOff <= nE),
  * and how many there are.  No output depends on any of this: the Philox counter
  * uses the original label (Q15).
  */

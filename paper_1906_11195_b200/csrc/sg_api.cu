@@ -457,7 +457,7 @@ extern "C" int sg_get_couplings(sg_sim *h, uint64_t *out)
         const SGHdr &hd = g.hdr[s];
         const uint32_t n = hd.counts & 63u;
         for (uint32_t j = 0; j < n; ++j) {
-            const uint32_t rp = g.rp_s[32 * s + j], xOff = rp & 255u, nX = (rp >> 16) & 31u;
+            const uint32_t rp = g.rp_s[32 * s + j], xOff = rp & 255u, nX = (rp >> 17) & 31u;
             const uint64_t p = (uint64_t)hd.pos0 + j;
             for (uint32_t r = 0; r < nX; ++r) {
                 const uint64_t nb = col[(uint64_t)hd.col_off + xOff + r], x = (uint64_t)hd.j_off + xOff + r;

@@ -386,7 +386,7 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t 
                 std::sort(keyT + ((g.gauge && par_e[i] != SG_NONE) ? 1 : 0), keyT + cT);
                 std::sort(keyX, keyX + cX);
                 g.orig_s[base + n] = i;
-                g.rp_s[base + n] = sX | sT << 8 | cX << 16 | cT << 21;          // tOff is made absolute below
+                g.rp_s[base + n] = sX | sT << 8 | cX << 17 | cT << 22;          // tOff is made absolute below
                 for (uint32_t q = 0; q < cT; ++q) rowT.push_back((uint32_t)(keyT[q] >> 32));
                 for (uint32_t q = 0; q < cX; ++q) { rowX.push_back((uint32_t)(keyX[q] >> 32)); rowXe.push_back((uint32_t)keyX[q]); }
                 shape = std::max(shape, sg_vb_shape(cX, cT));

@@ -43,8 +43,9 @@ Philox4 sg_philox_host(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint3
 //                      site by position), then its T entries in site order (parent first, then children by position);
 //                      the coupling array follows the X order, so entry e < nXs of the run has coupling j_off + e;
 //   orig_s[32 g + j] = original label of the j-th site of slice g (SG_NONE for j >= n): the Philox counter;
-//   rp_s[32 g + j]   = xOff | tOff << 8 | nX << 16 | nT << 21: where the site's X / T entries start inside the slice's
-//                      run (tOff counts from the start of the run, so tOff >= nXs), and how many there are.
+//   rp_s[32 g + j]   = xOff | tOff << 8 | nX << 17 | nT << 22: where the site's X / T entries start inside the slice's
+//                      run (tOff counts from the start of the run, so nXs <= tOff <= nE <= 256: nine bits), and how many
+//                      there are.
 // The kernels read a slice's run with one lane per ENTRY, 32 entries per step (every lane busy whatever the degrees,
 // streams coalesced, neighbouring entries gather from neighbouring words), park spin ^ coupling in shared memory, and
 // finish with one lane per SITE.

@@ -186,7 +186,7 @@ struct Streams {
 template <int G>
 __device__ __forceinline__ void count_unsatisfied(const uint64_t *sx, uint32_t rp, const Vec<G> &own, Planes<G> &P)
 {
-    const uint32_t xOff = rp & 255u, tOff = (rp >> 8) & 255u, nX = (rp >> 16) & 31u, nT = rp >> 21;
+    const uint32_t xOff = rp & 255u, tOff = (rp >> 8) & 511u, nX = (rp >> 17) & 31u, nT = rp >> 22;
     Vec<G> mT[4], mX[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
@@ -219,7 +219,7 @@ __device__ __forceinline__ void count_unsatisfied(const uint64_t *sx, uint32_t r
 template <int G, int NS>
 __device__ __forceinline__ void count_unsatisfied_short(const uint64_t *sx, uint32_t rp, const Vec<G> &own, Planes<G> &P)
 {
-    const uint32_t xOff = rp & 255u, tOff = (rp >> 8) & 255u, nX = (rp >> 16) & 31u, nT = rp >> 21;
+    const uint32_t xOff = rp & 255u, tOff = (rp >> 8) & 511u, nX = (rp >> 17) & 31u, nT = rp >> 22;
     Vec<G> mT[4], mX[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
@@ -342,7 +342,7 @@ __global__ void __launch_bounds__(SG_BT, MINB) k_vb_sweep(const __grid_constant_
 
     // flip <=> kk = d - 2u <= kstar <=> u >= ceil((d - kstar)/2); the slice's shape (warp-uniform) picks the count
     Planes<G> P;
-    const uint32_t d = ((rp >> 16) & 31u) + (rp >> 21), shape = h.counts >> 28;
+    const uint32_t d = ((rp >> 17) & 31u) + (rp >> 22), shape = h.counts >> 28;
     uint64_t any = 0;
     if (shape == 0) {
         count_unsatisfied_short<G, 2>(sx, rp, own, P);
@@ -443,7 +443,7 @@ k_init_vb_couplings(uint64_t *__restrict__ J, const uint64_t *__restrict__ eps, 
     const SGHdr h = hdr[slice];
     if (lane >= (h.counts & 63u)) return;
     const uint32_t rp = rp_s[slice * 32u + lane];
-    const uint32_t xOff = rp & 255u, nX = (rp >> 16) & 31u;
+    const uint32_t xOff = rp & 255u, nX = (rp >> 17) & 31u;
     const uint64_t p = (uint64_t)h.pos0 + lane;
     for (uint32_t r = 0; r < nX; ++r) {
         const uint64_t nb = col[(uint64_t)h.col_off + xOff + r];

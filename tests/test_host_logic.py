@@ -110,7 +110,7 @@ def _decode_rows(g):
                 continue
             p = pos0 + j
             label[p] = int(g["orig_s"][32 * s_ + j])
-            xOff, tOff, nX, nT = rp & 255, (rp >> 8) & 255, (rp >> 16) & 31, rp >> 21
+            xOff, tOff, nX, nT = rp & 255, (rp >> 8) & 511, (rp >> 17) & 31, rp >> 22
             assert tOff == t_run and xOff == x_run                 # site order, no gaps
             T[p] = [int(q) for q in g["col"][col_off + tOff:col_off + tOff + nT]]
             X[p] = [(int(g["col"][col_off + xOff + r]), int(j_off + xOff + r)) for r in range(nX)]
