@@ -220,7 +220,7 @@ void sg_host_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t
  * Slices: every class is cut greedily, in position order, into runs of at most 32 sites with at most 32*it entries of
  * which at most 32*itx are X entries; (it, itx) is chosen per class, from the class's degrees, among the budgets the
  * kernels are compiled for: for odd n_words (6,4) if its cut needs at most 30 % more slices than that of (8,6), else
- * (8,6); (4,3) for n_words = 2 mod 4; (4,2) for n_words = 0 mod 4.  Inside a class every window of 4096 sites is
+ * (8,6); (4,3) for even n_words (a thread then owns two words of its entry or site).  Inside a class every window of 4096 sites is
  * stably sorted by (demand, shape): demand 0 = a neighbour in a class of fewer than N/32 sites, 1 = fewer than N/8,
  * 2 = neither; shape 0 = at most 2 X and 2 T entries, 1 = at most 4 and 4, 2 = longer rows.  hdr[g] = 4 uint32: first
  * position, first index in col, first coupling entry, and n | nXs << 6 | nE << 16 | shape << 28 (sites, X entries, all entries, largest

@@ -339,8 +339,9 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t 
     };
     g.it_max = g.itx_max = 0;
     for (uint32_t k = 0; k < K; ++k) {
-        VBBudget best = n_words % 4 == 0 ? SG_VB_BUDGET_G4 : SG_VB_BUDGET_G2;
-        if (n_words % 2 != 0) {
+        const uint32_t G = sg_vb_group(n_words);
+        VBBudget best = G == 4 ? SG_VB_BUDGET_G4 : SG_VB_BUDGET_G2;
+        if (G == 1) {
             constexpr size_t NB = sizeof(SG_VB_BUDGETS_G1) / sizeof(SG_VB_BUDGETS_G1[0]);
             best = SG_VB_BUDGETS_G1[NB - 1];
             const uint64_t fewest = count_slices(k, best);
@@ -404,6 +405,18 @@ bool sg_build_vb_graph(int model, uint64_t N, double c, uint64_t seed, uint32_t 
     }
     g.hdr.push_back(SGHdr{(uint32_t)N, (uint32_t)g.col.size(), (uint32_t)g.jeid.size(), 0u});
     return true;
+}
+
+uint32_t sg_vb_group(uint32_t n_words)
+{
+    // two words (16-byte accesses) whenever n_words is even: measured 25-30 % faster than four words per thread, whose 96
+    // registers leave 20 warps per SM (profiles/r02_sweep.md)
+    uint32_t G = n_words % 2 == 0 ? 2u : 1u;
+    if (const char *e = std::getenv("SG_VB_G")) {
+        const uint32_t want = (uint32_t)std::atoi(e);
+        if ((want == 1 || want == 2 || want == 4) && n_words % want == 0) G = want;
+    }
+    return G;
 }
 
 // ---- host-only C entry points (include/sg.h) ------------------------------------------------------

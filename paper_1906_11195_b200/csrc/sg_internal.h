@@ -91,6 +91,9 @@ bool sg_build_vb_graph(int model /* SG_MODEL_VB or SG_MODEL_RRBG */, uint64_t N,
 struct VBBudget { uint32_t it, itx; };
 constexpr VBBudget SG_VB_BUDGETS_G1[] = {{6, 4}, {8, 6}};
 constexpr VBBudget SG_VB_BUDGET_G2 = {4, 3}, SG_VB_BUDGET_G4 = {4, 2};
+// words a thread of the sweep kernel owns for an instance of n_words words per site: 2 if n_words is even, else 1
+// (SG_VB_G=<1|2|4> chooses another divisor of n_words: a measurement knob; outputs are identical)
+uint32_t sg_vb_group(uint32_t n_words);
 
 std::vector<uint64_t> sg_vb_thresholds(double T, uint32_t dmax);   // thr[0..dmax], thr[0]=0
 std::vector<uint64_t> sg_sk_thresholds(double T, uint64_t N);      // thr[0..N-1]

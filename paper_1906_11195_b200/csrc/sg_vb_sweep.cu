@@ -10,8 +10,9 @@
 //   2. one lane per SITE: m_e = own ^ x_e (bit = bond unsatisfied), u = per-lane sum of the m_e in bit planes
 //      (carry-save adders), one Philox draw r per word shared by its 64 lanes, kstar = #{k >= 1 : r < thr[k]}, flip the
 //      lanes with u >= ceil((d - kstar)/2).  No floating point.
-// G = 4: a thread owns four words of its entry / site: one 32-byte sector per access (LDG.256) and one Philox call for
-// the four words (Q6).
+// G = 2 (even n_words): a thread owns two words of its entry / site: 16-byte accesses (LDG.128), one Philox call for the
+// two words (Q6).  G = 4 (32-byte accesses, LDG.256, one Philox call for four words) is kept behind SG_VB_G=4: at
+// 96 registers it is 25-30 % slower than G = 2.
 //
 // Memory behaviour (B200, profiles/): couplings, neighbour indices, labels and row pointers are read once per sweep,
 // coalesced, and stream through L2 (evict_first, no L1 allocation).  The gathers cost one L1TEX wavefront per distinct
@@ -522,7 +523,7 @@ int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint64_t N, uint64_t
 {
     if (c.n == 0) return SG_OK;
     const bool wide = force_wide() || N * W >= (1ull << 32) || nJ * W >= (1ull << 32);
-    const uint32_t G = (W % 4 == 0) ? 4 : (W % 2 == 0) ? 2 : 1;
+    const uint32_t G = sg_vb_group(W);
     if (c.nslices * (uint64_t)(W / G) >= (1ull << 31)) { sg_set_error("sgk_vb_sweep_class: class too large"); return SG_EINVAL; }
     if (G != 1 && (c.it > 4 || c.itx > (G == 2 ? 3u : 2u))) { sg_set_error("k_vb_sweep: the slice budget of the class exceeds the kernels'"); return SG_EINVAL; }
     if (!wide) {

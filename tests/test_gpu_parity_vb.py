@@ -221,8 +221,8 @@ def test_relabelling_does_not_change_any_output(sg, oracle_mod, monkeypatch, ord
 
 @pytest.mark.parametrize("knob,value", [("SG_VB_IT", "6"), ("SG_VB_IT", "8"), ("SG_VB_WIN", "0"), ("SG_VB_WIN", "64"),
                                         ("SG_VB_DEMAND", "0"), ("SG_VB_GAUGE", "0"), ("SG_VB_SLACK", "100"),
-                                        ("SG_VB_CARVEOUT", "50"), ("SG_NO_PDL", "1")])
-@pytest.mark.parametrize("N,c,T,seed,W", [(20000, 4.0, 1.0, 21, 1), (3000, 9.0, 0.6, 22, 3)])
+                                        ("SG_VB_CARVEOUT", "50"), ("SG_NO_PDL", "1"), ("SG_VB_G", "4"), ("SG_VB_G", "1")])
+@pytest.mark.parametrize("N,c,T,seed,W", [(20000, 4.0, 1.0, 21, 1), (3000, 9.0, 0.6, 22, 3), (5000, 4.0, 1.0, 23, 4)])
 def test_layout_and_launch_knobs_change_no_output(sg, oracle_mod, monkeypatch, knob, value, N, c, T, seed, W):
     """The measurement knobs of DESIGN.md section 10 choose among layouts and launch configurations (entry budget of a
     slice, hence the kernel instantiation; window of the (demand, shape) sort; gauge fixing; shared-memory carve-out;

@@ -210,7 +210,7 @@ def test_host_generator_matches_oracle_and_layout_is_consistent(sg, oracle_mod, 
             runs.append((p, n, sX, sE))
             p += n
         return runs
-    budgets = [(6, 4), (8, 6)] if W % 2 else [(4, 3)] if W % 4 else [(4, 2)]
+    budgets = [(6, 4), (8, 6)] if W % 2 else [(4, 3)]
     hdr = g["hdr"].astype(np.int64)
     s_ = 0
     for k in range(K):
