@@ -108,6 +108,23 @@ int sg_snapshot(sg_sim *h, uint32_t slot);
 int sg_correlation(sg_sim *h, uint32_t slot, uint64_t *out_counts);
 
 /*
+ * sg_correlation_noalloc -- sg_correlation for callers that cannot allocate device memory (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): the same counts D_l, exact integers, with the
+ * kernel's per-lane counters in a static device array of the library instead of a buffer of the handle.  The call makes no
+ * cudaMalloc / cudaFree and calls no allocating routine.
+ *   h           a handle of a graph model (VB, RRBG, RRG) with n_words <= sg_noalloc_max_words() = 64; beyond that
+ *               SG_EINVAL with a message that names the limit (the array is 64 * 64 counters = 32 KiB, held by every GPU
+ *               that loads the library until exit);
+ *   slot        written by sg_snapshot before (SG_ESLOT otherwise; sg_snapshot allocates a slot on its first use, so
+ *               write every slot at set-up);
+ *   out_counts  HOST, 64*n_words uint64.
+ * All handles and all calls share the one array; it is cleared at the start of every call.  Calls that overlap on the GPU
+ * (different streams or host threads) race: serialise them.  Synchronises the stream.
+ */
+int sg_correlation_noalloc(sg_sim *h, uint32_t slot, uint64_t *out_counts);
+uint32_t sg_noalloc_max_words(void);
+
+/*
  * sg_energy -- per-lane energy of the current configuration, exact integers.
  *   VB: out[l] = E_l  = -sum_{(ij) in E} J_ij s_i s_j
  *   SK: out[l] = E'_l = -sum_{i<j} J'_ij s_i s_j with J' = +-1; energy = E'_l / sqrt(N)

@@ -26,6 +26,8 @@ SYMBOLS = {
     "sg_sweep": (C.c_int, [_vp, _u64]),
     "sg_snapshot": (C.c_int, [_vp, _u32]),
     "sg_correlation": (C.c_int, [_vp, _u32, _vp]),
+    "sg_correlation_noalloc": (C.c_int, [_vp, _u32, _vp]),
+    "sg_noalloc_max_words": (_u32, []),
     "sg_energy": (C.c_int, [_vp, _vp]),
     "sg_corr_configure": (C.c_int, [_vp, _u32]),
     "sg_corr_accumulate": (C.c_int, [_vp, _u32, _vp, _vp]),
@@ -146,6 +148,16 @@ def sg_correlation(h: int, slot: int, out_counts: np.ndarray) -> np.ndarray:
     return out_counts
 
 
+def sg_correlation_noalloc(h: int, slot: int, out_counts: np.ndarray) -> np.ndarray:
+    assert out_counts.dtype == np.uint64 and out_counts.flags.c_contiguous
+    _check(load_library().sg_correlation_noalloc(h, int(slot), _ptr(out_counts)))
+    return out_counts
+
+
+def sg_noalloc_max_words() -> int:
+    return int(load_library().sg_noalloc_max_words())
+
+
 def sg_energy(h: int, out: np.ndarray) -> np.ndarray:
     assert out.dtype == np.int64 and out.flags.c_contiguous
     _check(load_library().sg_energy(h, _ptr(out)))
@@ -199,6 +211,11 @@ class Sim:
     def correlation(self, slot: int, out: np.ndarray | None = None) -> np.ndarray:
         out = np.zeros(self.lanes, dtype=np.uint64) if out is None else out
         return sg_correlation(self._h, slot, out)
+
+    def correlation_noalloc(self, slot: int, out: np.ndarray | None = None) -> np.ndarray:
+        """sg_correlation_noalloc: the same counts with the kernel's counters in the library's static device array."""
+        out = np.zeros(self.lanes, dtype=np.uint64) if out is None else out
+        return sg_correlation_noalloc(self._h, slot, out)
 
     def energy(self, out: np.ndarray | None = None) -> np.ndarray:
         out = np.zeros(self.lanes, dtype=np.int64) if out is None else out

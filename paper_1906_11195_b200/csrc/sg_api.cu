@@ -279,6 +279,19 @@ extern "C" int sg_correlation(sg_sim *h, uint32_t slot, uint64_t *out_counts)
     return SG_OK;
 }
 
+// sg_correlation for callers that must not allocate: the counters live in the library's static device array
+extern "C" uint32_t sg_noalloc_max_words(void) { return SG_NOALLOC_MAX_WORDS; }
+
+extern "C" int sg_correlation_noalloc(sg_sim *h, uint32_t slot, uint64_t *out_counts)
+{
+    if (!h || !out_counts) { sg_set_error("sg_correlation_noalloc: null argument"); return SG_EINVAL; }
+    if (!on_own_device(h, "sg_correlation_noalloc")) return SG_EINVAL;
+    if (h->model != SG_MODEL_VB) { sg_set_error("sg_correlation_noalloc: graph models only (VB, RRBG, RRG)"); return SG_EINVAL; }
+    if (slot >= SG_MAX_SLOTS) { sg_set_error("sg_correlation_noalloc: slot out of range"); return SG_EINVAL; }
+    if (!h->slot[slot]) { sg_set_error("sg_correlation_noalloc: slot was never written"); return SG_ESLOT; }
+    return sgk_xor_popcount_noalloc(current_config(h), h->slot[slot], h->g.N, h->W, out_counts, sgx_stream());
+}
+
 // ---- windowed protocol: device-side accumulation of correlation counts ---------------------
 extern "C" int sg_corr_configure(sg_sim *h, uint32_t nbins)
 {

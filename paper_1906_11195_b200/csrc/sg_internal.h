@@ -124,6 +124,9 @@ int sgk_vb_sweep_class(const VBDevice &d, const VBClass &c, uint64_t N, uint64_t
                        bool reverse, cudaStream_t st);
 // counts[64*W] (device, u64) += per-lane number of set bits of (a XOR b) over n_sites*W words
 int sgk_xor_popcount(const uint64_t *a, const uint64_t *b, uint64_t n_sites, uint32_t W, uint64_t *counts, cudaStream_t st);
+// the same with the counters in the library's static device array (no allocation anywhere); out_host: HOST, 64*W uint64
+constexpr uint32_t SG_NOALLOC_MAX_WORDS = 64;
+int sgk_xor_popcount_noalloc(const uint64_t *a, const uint64_t *b, uint64_t n_sites, uint32_t W, uint64_t *out_host, cudaStream_t st);
 // the same against up to 3 stored configurations in one pass: counts[s][64*W] += D(a, b[s])
 int sgk_xor_popcount_multi(const uint64_t *a, const uint64_t *const *b, uint32_t n, uint64_t n_sites, uint32_t W, uint64_t *const *counts,
                            cudaStream_t st);

@@ -5,6 +5,7 @@
 
 #include <algorithm>
 #include <atomic>
+#include <string>
 
 #include "sg_device.cuh"
 #include "sg_internal.h"
@@ -114,6 +115,42 @@ int sgk_xor_popcount(const uint64_t *a, const uint64_t *b, uint64_t n_sites, uin
         k_xor_popcount<false><<<grid, 256, 0, st>>>(a, b, n_sites, W, (unsigned long long *)counts);
     }
     SG_LAUNCH_CHECK();
+    return SG_OK;
+}
+
+// ------------------------------------------------------------------------------------ correlation without allocation
+// sg_correlation_noalloc (include/sg.h): the per-lane counters that k_xor_popcount adds to live in a file-scope device
+// array instead of a buffer of the handle.  Every GPU that loads the library holds these 32 KiB until exit.  In host code
+// the array's NAME is a host-side stand-in, not a device address: its address on the current device comes from
+// cudaGetSymbolAddress, once per device with that device current.  All calls share the array: it is cleared at the start of
+// each call, and calls that overlap on the GPU (other streams, other host threads) race.
+static __device__ __align__(256) unsigned long long g_noalloc_counts[64 * SG_NOALLOC_MAX_WORDS];
+
+int sgk_xor_popcount_noalloc(const uint64_t *a, const uint64_t *b, uint64_t n_sites, uint32_t W, uint64_t *out_host, cudaStream_t st)
+{
+    if (W == 0 || W > SG_NOALLOC_MAX_WORDS) {
+        sg_set_error("sg_correlation_noalloc: n_words exceeds the static scratch (at most " + std::to_string(SG_NOALLOC_MAX_WORDS) + " words per site)");
+        return SG_EINVAL;
+    }
+    constexpr int MAX_DEV = 64;
+    static unsigned long long *addr[MAX_DEV] = {nullptr};     // the array's device address, per device
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEV) { sg_set_error("sg_correlation_noalloc: no usable current device"); return SG_ECUDA; }
+    if (!addr[dev]) {
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_counts);
+        if (e != cudaSuccess || !p) { sg_set_error(std::string("sg_correlation_noalloc: cudaGetSymbolAddress failed: ") + cudaGetErrorString(e)); return SG_ECUDA; }
+        addr[dev] = static_cast<unsigned long long *>(p);
+    }
+    unsigned long long *counts = addr[dev];
+    const size_t bytes = (size_t)64 * W * sizeof(unsigned long long);
+    cudaError_t e = cudaMemsetAsync(counts, 0, bytes, st);      // the array keeps the last call's counts
+    if (e != cudaSuccess) { sg_set_error(std::string("sg_correlation_noalloc: ") + cudaGetErrorString(e)); return SG_ECUDA; }
+    const int rc = sgk_xor_popcount(a, b, n_sites, W, reinterpret_cast<uint64_t *>(counts), st);
+    if (rc) return rc;
+    e = cudaMemcpyAsync(out_host, counts, bytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { sg_set_error(std::string("sg_correlation_noalloc: ") + cudaGetErrorString(e)); return SG_ECUDA; }
     return SG_OK;
 }
 
